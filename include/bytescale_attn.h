@@ -1,0 +1,196 @@
+/* bytescale_attn.h — C-ABI boundary of the B200-native ByteScale attention hot path.
+ *
+ * What this library is: the per-device data-parallel hot path of one Hybrid Data Parallelism
+ * (HDP) rank of ByteScale (arXiv 2502.21231; PAPER.md = /root/reference/PAPER.md):
+ * causal self-attention over a packed buffer of variable-length documents ("packing ... employs
+ * a special segmented attention mask to ensure that each sequence is processed independently",
+ * PAPER.md:93) in which some sequences are whole and others are zigzag context-parallel shards
+ * ("each subsequence ... is uniformly divided into 2N parts and symmetrically assigned to the N
+ * devices"), computed one Q-chunk x KV-chunk ring step at a time,
+ * each step returning a partial O and a per-row natural-log LSE; a separate LSE merge; and the
+ * matching backward.  BASELINE.json north_star fixes the call list.
+ *
+ * Conventions for every entry point
+ *   - extern "C"; plain pointers and sizes; no exception crosses the boundary; nothing prints.
+ *   - Every function returning bs_status_t returns BS_OK (0) or a negative code; the detail text
+ *     is available from bs_last_error() (thread-local, valid until the next call on the thread).
+ *   - "device" pointers are CUDA device memory owned by the caller; "host" pointers are ordinary
+ *     host memory.  The library never allocates or frees device memory, and never synchronises
+ *     the device: all device work is enqueued on `stream` (a cudaStream_t passed as void*; NULL =
+ *     the legacy default stream).  Host arrays may be freed as soon as the call returns.
+ *   - Tensors: Q, O, dO, dQ are [q_rows][n_q_heads][head_dim] bf16 with dim stride 1, head stride
+ *     head_dim and row stride q_row_stride elements.  K, V, dK, dV are
+ *     [kv_rows][n_kv_heads][head_dim] bf16 with row stride kv_row_stride.  LSE and delta are fp32,
+ *     element (h, row) at [h * lse_head_stride + row].  dQ_acc is fp32 [q_rows][n_q_heads][head_dim]
+ *     densely packed.  Base pointers must be 16-byte aligned, row strides multiples of 8 elements.
+ *   - head_dim in {64, 128}; n_q_heads % n_kv_heads == 0 (GQA).
+ */
+#ifndef BYTESCALE_ATTN_H_
+#define BYTESCALE_ATTN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BS_VERSION 100 /* 0.1.0 */
+
+typedef enum {
+  BS_OK = 0,
+  BS_ERR_INVALID_ARG = -1, /* null pointer, bad range, bad stride, inconsistent segments */
+  BS_ERR_UNSUPPORTED = -2, /* head_dim not in {64,128}, device is not sm_100 */
+  BS_ERR_WORKSPACE = -3,   /* workspace null / too small / misaligned */
+  BS_ERR_CUDA = -4,        /* a CUDA runtime/driver call failed; text from cudaGetErrorString */
+  BS_ERR_HOST_OOM = -5
+} bs_status_t;
+
+const char* bs_status_string(bs_status_t s); /* static storage */
+const char* bs_last_error(void);             /* thread-local detail of the last failure */
+int bs_version(void);
+
+/* ------------------------------------------------------------------------------------------ */
+/* Planning — host only, integers only.  Data-aware sharding, device-local view:               */
+/* "each sequence is processed by the minimal number of ranks"; long sequences   */
+/* are zigzag-split 2N ways, rank r holding parts r and 2N-1-r; KV chunks arrive  */
+/* in ring order.  Canonical form:            */
+/*   parts   : cp == 1 -> one part [0,len); cp == N >= 2 -> part k = [floor(k*len/2N),           */
+/*             floor((k+1)*len/2N)), k in [0,2N); rank p holds part p ("low") and 2N-1-p ("high") */
+/*   Q buffer: sequences in input order, low part rows then high part rows                      */
+/*   steps   : n_steps = max cp; at step s the sequences with cp > s take part, source rank      */
+/*             p = (rank - s) mod cp; the step's KV buffer = [low part of p ; high part of p]    */
+/*             per participating sequence, in input order                                       */
+/*   segments: per participating sequence, for q part in (low, high), for k part in (low, high): */
+/*             emitted iff both parts are non-empty and at least one pair is visible;            */
+/*             causal_offset = q_part_global_start - k_part_global_start (unclamped)             */
+/* ------------------------------------------------------------------------------------------ */
+
+typedef struct {
+  int32_t len;  /* full sequence length in tokens, >= 1 */
+  int32_t cp;   /* context-parallel degree N of this sequence; 1 = whole on this device */
+  int32_t rank; /* this device's rank inside the sequence's CP group, 0 <= rank < cp */
+} bs_seq_t;
+
+/* One rectangular piece of attention work: queries = rows [q_begin,q_end) of the Q-side buffers,
+ * keys = rows [k_begin,k_end) of THIS call's K/V buffers.  With a, b the 0-based indices inside
+ * the two ranges, key b is visible to query a iff  b <= a + causal_offset.
+ * Two segments of one call have identical or disjoint q ranges; a row's softmax runs over the
+ * union of the visible keys of every segment that contains the row. */
+typedef struct {
+  int32_t q_begin, q_end;
+  int32_t k_begin, k_end;
+  int32_t causal_offset;
+  int32_t seq; /* index into the planner's input seqs[] (informational for device calls) */
+} bs_seg_t;
+
+typedef struct {
+  int32_t step;               /* ring step index s */
+  int32_t n_segs;
+  const bs_seg_t* segs;       /* [n_segs], owned by the plan */
+  int32_t kv_rows;            /* rows of this step's K/V buffer */
+  int32_t n_kv_seqs;          /* sequences present in this step's K/V buffer */
+  const int32_t* kv_seq;      /* [n_kv_seqs] sequence indices, input order */
+  const int32_t* kv_src_rank; /* [n_kv_seqs] CP rank whose K/V this is: (rank - s) mod cp */
+  const int32_t* cu_rows_k;   /* [n_kv_seqs + 1] first K/V row of each present sequence */
+  int64_t visible_pairs;      /* visible (query,key) pairs of the step, per head */
+} bs_step_t;
+
+typedef struct bs_plan bs_plan_t; /* opaque, host memory owned by the library */
+
+/* Build the plan for this device.  seqs: host, [n_seqs].  *out receives a plan to be released
+ * with bs_plan_destroy.  Errors: INVALID_ARG (null, n_seqs < 0, len < 1, cp < 1, rank out of
+ * range, total rows > INT32_MAX), HOST_OOM. */
+bs_status_t bs_plan(const bs_seq_t* seqs, int32_t n_seqs, bs_plan_t** out);
+
+/* Convenience form of north_star's "per-sequence lengths and a CP degree": sequences with
+ * len >= min_shard_len get (cp, rank); all others cp = 1, rank = 0. */
+bs_status_t bs_plan_uniform(const int32_t* lens, int32_t n, int32_t cp, int32_t rank,
+                            int32_t min_shard_len, bs_plan_t** out);
+
+int32_t bs_plan_n_seqs(const bs_plan_t* p);
+int32_t bs_plan_q_rows(const bs_plan_t* p);           /* rows of the local Q-side buffers */
+const int32_t* bs_plan_cu_rows_q(const bs_plan_t* p); /* [n_seqs + 1] first local row per seq */
+/* Global position (0-based inside its sequence) and sequence index of every local Q row:
+ * [q_rows] each.  Owned by the plan. */
+const int32_t* bs_plan_q_pos(const bs_plan_t* p);
+const int32_t* bs_plan_q_seq(const bs_plan_t* p);
+int32_t bs_plan_n_steps(const bs_plan_t* p); /* max cp over the input (0 if n_seqs == 0) */
+const bs_step_t* bs_plan_step(const bs_plan_t* p, int32_t s); /* NULL if s out of range */
+void bs_plan_destroy(bs_plan_t* p);                           /* NULL is a no-op */
+
+/* ------------------------------------------------------------------------------------------ */
+/* Device calls                                                                                */
+/* ------------------------------------------------------------------------------------------ */
+
+typedef struct {
+  int32_t n_q_heads, n_kv_heads, head_dim;
+  float softmax_scale;   /* <= 0 means 1/sqrt(head_dim) */
+  int32_t q_rows;        /* rows in Q/O/dO/dQ/LSE/delta buffers of this call */
+  int32_t kv_rows;       /* rows in K/V/dK/dV buffers of this call */
+  int64_t q_row_stride;  /* elements */
+  int64_t kv_row_stride; /* elements */
+  int64_t lse_head_stride; /* elements; >= q_rows */
+} bs_attn_shape_t;
+
+/* Bytes of caller-owned device workspace a forward (bwd == 0) or backward (bwd != 0) call with
+ * n_segs segments needs.  The workspace must be 256-byte aligned.  It holds the uploaded
+ * segment/work-item tables and the scheduler's counters; its content is dead after the call's
+ * kernels finish, and one workspace must not be shared by calls in flight on different streams. */
+bs_status_t bs_attn_workspace_bytes(const bs_attn_shape_t* shape, int32_t n_segs, int bwd,
+                                    size_t* bytes);
+
+/* Forward of one Q-chunk x KV-chunk step (flash attention = exact attention,
+ * PAPER.md:97).  For every head h and every row i in [out_row_begin, out_row_end):
+ *   S_ij = scale * q_i . k_j over the visible keys j of every segment containing row i
+ *   LSE[h,i] = ln sum_j exp(S_ij)   (natural log; -inf if no key is visible)
+ *   O[i,h,:] = sum_j exp(S_ij - LSE[h,i]) * V[j, h / (Hq/Hkv), :]   (0 if no key is visible)
+ * Rows of the range covered by no segment get O = 0, LSE = -inf.  Rows outside the range are
+ * not written.  Q,K,V,O: device bf16.  LSE: device fp32.  segs: host.  ws: device. */
+bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void* K, const void* V,
+                        const bs_seg_t* segs, int32_t n_segs, int32_t out_row_begin,
+                        int32_t out_row_end, void* O, float* LSE, void* ws, size_t ws_bytes,
+                        void* stream);
+
+/* Backward preparation (a5): delta[h,i] = sum_d dO[i,h,d] * O_final[i,h,d] for all q_rows, and
+ * dQ_acc = 0.  O_final is the MERGED output.  All device pointers. */
+bs_status_t bs_attn_bwd_prep(const bs_attn_shape_t* shape, const void* O_final, const void* dO,
+                             float* delta, float* dQ_acc, void* stream);
+
+/* Backward of one step (a6), using the MERGED LSE and delta so that each step yields the exact
+ * partial gradients (reading 13):
+ *   P_ij = exp(S_ij - LSE_final[h,i]);  dP_ij = dO_i . v_j;  dS_ij = P_ij * (dP_ij - delta[h,i])
+ *   dV[j,g,:] = sum_{h in g} sum_i P_ij dO[i,h,:]        (overwritten; unreferenced rows = 0)
+ *   dK[j,g,:] = scale * sum_{h in g} sum_i dS_ij Q[i,h,:] (overwritten; unreferenced rows = 0)
+ *   dQ_acc[i,h,:] += scale * sum_j dS_ij K[j,g,:]         (fp32, accumulated across steps)
+ * All kv_rows rows of dK and dV are written. */
+bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, const void* K, const void* V,
+                        const void* dO, const float* LSE_final, const float* delta,
+                        const bs_seg_t* segs, int32_t n_segs, float* dQ_acc, void* dK, void* dV,
+                        void* ws, size_t ws_bytes, void* stream);
+
+/* a7: dQ = bf16(dQ_acc) for all q_rows (round to nearest even). */
+bs_status_t bs_attn_bwd_finish(const bs_attn_shape_t* shape, const float* dQ_acc, void* dQ,
+                               void* stream);
+
+/* LSE merge (a4) of n_parts partial results over rows [row_begin,row_end), every head:
+ *   M = max_s LSE_s; all -inf -> O = 0, LSE = -inf; else
+ *   w_s = exp(LSE_s - M), Z = sum_s w_s, LSE = M + ln Z, O = sum_s (w_s / Z) O_s.
+ * O_parts / LSE_parts: HOST arrays of n_parts DEVICE pointers, each laid out per `shape`
+ * (q_rows, q_row_stride, lse_head_stride).  O_out may alias O_parts[k] and LSE_out may alias
+ * LSE_parts[k] (running merge).  1 <= n_parts <= BS_MAX_MERGE_PARTS. */
+#define BS_MAX_MERGE_PARTS 64
+bs_status_t bs_lse_merge(int32_t n_parts, const void* const* O_parts,
+                         const float* const* LSE_parts, const bs_attn_shape_t* shape,
+                         int32_t row_begin, int32_t row_end, void* O_out, float* LSE_out,
+                         void* stream);
+
+/* Number of kernels this library has launched on the calling thread since the last reset
+ * (bench.py's "gpu_launches"). */
+int64_t bs_launch_count(void);
+void bs_launch_count_reset(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BYTESCALE_ATTN_H_ */
