@@ -96,7 +96,7 @@ typedef struct {
   int64_t visible_pairs;      /* visible (query,key) pairs of the step, per head */
 } bs_step_t;
 
-typedef struct bs_plan bs_plan_t; /* opaque, host memory owned by the library */
+typedef struct bs_plan_s bs_plan_t; /* opaque, host memory owned by the library */
 
 /* Build the plan for this device.  seqs: host, [n_seqs].  *out receives a plan to be released
  * with bs_plan_destroy.  Errors: INVALID_ARG (null, n_seqs < 0, len < 1, cp < 1, rank out of
@@ -117,6 +117,9 @@ const int32_t* bs_plan_q_pos(const bs_plan_t* p);
 const int32_t* bs_plan_q_seq(const bs_plan_t* p);
 int32_t bs_plan_n_steps(const bs_plan_t* p); /* max cp over the input (0 if n_seqs == 0) */
 const bs_step_t* bs_plan_step(const bs_plan_t* p, int32_t s); /* NULL if s out of range */
+/* Global position / sequence index of every row of step s's K/V buffer: [kv_rows] each. */
+const int32_t* bs_plan_step_k_pos(const bs_plan_t* p, int32_t s);
+const int32_t* bs_plan_step_k_seq(const bs_plan_t* p, int32_t s);
 void bs_plan_destroy(bs_plan_t* p);                           /* NULL is a no-op */
 
 /* ------------------------------------------------------------------------------------------ */

@@ -1,0 +1,34 @@
+// launch_utils.h — host-side helpers shared by the library's .cu files: shape validation,
+// the uncovered-row fill launch, and TMA tensor-map creation through the driver entry point
+// (so the library links against cudart only).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "common.h"
+
+namespace bs {
+
+bs_status_t validate_shape(const bs_attn_shape_t* s, const char* who);
+
+// Zero rows [begin,end) of up to two [row][head][D] bf16 tensors and set lse[h][row] = -inf for
+// each (begin,end) pair in the device array d_ranges.  max_rows = longest range (grid sizing).
+bs_status_t launch_fill_rows(const int2* d_ranges, int n_ranges, int64_t max_rows, void* A, void* B,
+                             float* lse, int n_heads, int head_dim, int64_t row_stride,
+                             int64_t lse_head_stride, cudaStream_t st);
+
+// 3-D tensor map over a [rows][heads][head_dim] tensor (innermost first: dim, head, row).
+//   elem_bytes 2 (bf16) or 4 (fp32); box = (box_dim, 1, box_rows); swizzle128: 128-byte swizzle
+//   (box_dim * elem_bytes must be 128) or none.
+bs_status_t make_tensor_map_3d(CUtensorMap* map, const void* base, int elem_bytes, int head_dim,
+                               int n_heads, int64_t rows, int64_t row_stride_elems, int box_dim,
+                               int box_rows, bool swizzle128);
+
+}  // namespace bs
+
+#include "worklist.h"
+namespace bs {
+bs_status_t upload_tables(const SchedTables& tb, void* ws, size_t ws_bytes, cudaStream_t st,
+                          WsLayout* layout);
+int sm_count();
+}  // namespace bs

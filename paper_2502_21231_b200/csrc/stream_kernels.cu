@@ -1,0 +1,363 @@
+// stream_kernels.cu — the HBM-bound kernels of the path: bs_lse_merge (a4), bs_attn_bwd_prep
+// (a5), bs_attn_bwd_finish (a7) and the row-fill helper used by fwd/bwd for uncovered rows.
+//
+// All of them stream [row][head][D] bf16 tensors with 128-bit accesses; none has data reuse
+// beyond the per-(row,head) LSE weights, so the roofline is HBM bandwidth:
+//   merge : (n + 1) * rows * Hq * (2 D + 4) bytes
+//   prep  : rows * Hq * (2 * 2 D read + 4 + 4 D written)
+//   finish: rows * Hq * (4 D read + 2 D written)
+// Layout trick shared by merge and prep: a block owns a tile of kRowsPerTile consecutive rows x a
+// slab of heads, so that the fp32 [head][row] arrays (LSE, delta) are touched in full 32-byte
+// sectors by one block, while the O stream is walked in memory order.
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <math_constants.h>
+
+#include "common.h"
+#include "launch_utils.h"
+
+namespace {
+
+constexpr int kRowsPerTile = 8;     // 8 fp32 LSE values of one head = one 32-byte sector
+constexpr int kStreamThreads = 256;
+
+struct MergeParams {
+  const uint4* O_parts[BS_MAX_MERGE_PARTS];
+  const float* LSE_parts[BS_MAX_MERGE_PARTS];
+  uint4* O_out;
+  float* LSE_out;
+  int n_parts, n_heads, heads_per_block, row_begin, row_end;
+  int64_t row_stride_v;  // q_row_stride in uint4 (8 bf16) units
+  int64_t lse_head_stride;
+};
+
+__device__ __forceinline__ uint4 ldg_stream(const uint4* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void stg_stream(uint4* p, const uint4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x),
+               "r"(v.y), "r"(v.z), "r"(v.w)
+               : "memory");
+}
+__device__ __forceinline__ void fma_bf16x8(float (&acc)[8], const uint4& v, float w) {
+  const uint32_t u[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    acc[2 * i] = fmaf(w, __uint_as_float(u[i] << 16), acc[2 * i]);
+    acc[2 * i + 1] = fmaf(w, __uint_as_float(u[i] & 0xffff0000u), acc[2 * i + 1]);
+  }
+}
+__device__ __forceinline__ uint32_t pack2(float lo, float hi) {
+  __nv_bfloat162 t = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&t);
+}
+
+// grid: (row tiles, head slabs).  smem: weights[n_parts][kRowsPerTile][heads_per_block] fp32.
+template <int kVecPerHead>  // uint4 per (row, head): D / 8
+__global__ void __launch_bounds__(kStreamThreads) lse_merge_kernel(const __grid_constant__ MergeParams p) {
+  extern __shared__ float w_smem[];
+  const int row0 = p.row_begin + blockIdx.x * kRowsPerTile;
+  const int h0 = blockIdx.y * p.heads_per_block;
+  const int nh = min(p.heads_per_block, p.n_heads - h0);
+  const int nrows = min(kRowsPerTile, p.row_end - row0);
+  const int n = p.n_parts;
+
+  // phase 1: weights.  thread -> (head, row) with row fastest: one 32 B LSE sector per 8 threads.
+  for (int t = threadIdx.x; t < nh * kRowsPerTile; t += blockDim.x) {
+    const int r = t % kRowsPerTile, h = t / kRowsPerTile;
+    if (r >= nrows) continue;
+    const int64_t off = (int64_t)(h0 + h) * p.lse_head_stride + (row0 + r);
+    float M = -CUDART_INF_F;
+    for (int s = 0; s < n; ++s) M = fmaxf(M, __ldg(p.LSE_parts[s] + off));
+    float Z = 0.f;
+    if (M != -CUDART_INF_F)
+      for (int s = 0; s < n; ++s) Z += __expf(__ldg(p.LSE_parts[s] + off) - M);
+    const float invZ = (M == -CUDART_INF_F) ? 0.f : 1.f / Z;
+    for (int s = 0; s < n; ++s) {
+      const float l = __ldg(p.LSE_parts[s] + off);
+      w_smem[(s * kRowsPerTile + r) * p.heads_per_block + h] =
+          (M == -CUDART_INF_F) ? 0.f : __expf(l - M) * invZ;
+    }
+    p.LSE_out[off] = (M == -CUDART_INF_F) ? -CUDART_INF_F : M + __logf(Z);
+  }
+  __syncthreads();
+
+  // phase 2: stream O.  Within a row the slab's heads are contiguous: nh * kVecPerHead uint4.
+  const int vec_per_row = nh * kVecPerHead;
+  for (int t = threadIdx.x; t < nrows * vec_per_row; t += blockDim.x) {
+    const int r = t / vec_per_row, c = t % vec_per_row;
+    const int h = c / kVecPerHead;
+    const int64_t off = (int64_t)(row0 + r) * p.row_stride_v + (int64_t)h0 * kVecPerHead + c;
+    float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    for (int s0 = 0; s0 < n; s0 += 8) {
+      uint4 v[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j)
+        if (s0 + j < n) v[j] = ldg_stream(p.O_parts[s0 + j] + off);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        if (s0 + j < n) {
+          const float w = w_smem[((s0 + j) * kRowsPerTile + r) * p.heads_per_block + h];
+          // a part with zero weight (LSE = -inf) may hold anything, including NaN: skip it
+          if (w != 0.f) fma_bf16x8(acc, v[j], w);
+        }
+      }
+    }
+    uint4 o;
+    o.x = pack2(acc[0], acc[1]);
+    o.y = pack2(acc[2], acc[3]);
+    o.z = pack2(acc[4], acc[5]);
+    o.w = pack2(acc[6], acc[7]);
+    stg_stream(p.O_out + off, o);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// bwd_prep: delta[h,row] = sum_d dO * O ; dQ_acc = 0.  Same tiling as the merge.
+// ------------------------------------------------------------------------------------------------
+struct PrepParams {
+  const uint4* O;
+  const uint4* dO;
+  float* delta;
+  float4* dQ_acc;
+  int n_heads, heads_per_block, rows;
+  int64_t row_stride_v, lse_head_stride;
+};
+
+template <int kVecPerHead>
+__global__ void __launch_bounds__(kStreamThreads) bwd_prep_kernel(const __grid_constant__ PrepParams p) {
+  extern __shared__ float d_smem[];  // [kRowsPerTile][heads_per_block]
+  const int row0 = blockIdx.x * kRowsPerTile;
+  const int h0 = blockIdx.y * p.heads_per_block;
+  const int nh = min(p.heads_per_block, p.n_heads - h0);
+  const int nrows = min(kRowsPerTile, p.rows - row0);
+  const int vec_per_row = nh * kVecPerHead;
+  // kVecPerHead (8 or 16) consecutive lanes share one (row, head); the loop trip count is
+  // uniform per block so that the shuffles always see a full warp
+  const int total = nrows * vec_per_row;
+  for (int base = 0; base < total; base += blockDim.x) {
+    const int t = base + threadIdx.x;
+    const bool valid = t < total;
+    const int r = valid ? t / vec_per_row : 0, c = valid ? t % vec_per_row : 0;
+    const int h = c / kVecPerHead;
+    const int64_t off = (int64_t)(row0 + r) * p.row_stride_v + (int64_t)h0 * kVecPerHead + c;
+    float s = 0.f;
+    if (valid) {
+      const uint4 a = ldg_stream(p.O + off), b = ldg_stream(p.dO + off);
+      const uint32_t ua[4] = {a.x, a.y, a.z, a.w}, ub[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        s = fmaf(__uint_as_float(ua[i] << 16), __uint_as_float(ub[i] << 16), s);
+        s = fmaf(__uint_as_float(ua[i] & 0xffff0000u), __uint_as_float(ub[i] & 0xffff0000u), s);
+      }
+    }
+#pragma unroll
+    for (int m = kVecPerHead / 2; m >= 1; m >>= 1) s += __shfl_xor_sync(0xffffffffu, s, m);
+    if (valid) {
+      if ((c % kVecPerHead) == 0) d_smem[r * p.heads_per_block + h] = s;
+      // zero the fp32 accumulator: 2 float4 per bf16 uint4
+      float4* dq = p.dQ_acc + (((int64_t)(row0 + r) * p.n_heads + h0) * kVecPerHead + c) * 2;
+      dq[0] = make_float4(0.f, 0.f, 0.f, 0.f);
+      dq[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  }
+  __syncthreads();
+  for (int t = threadIdx.x; t < nh * kRowsPerTile; t += blockDim.x) {
+    const int r = t % kRowsPerTile, h = t / kRowsPerTile;
+    if (r < nrows)
+      p.delta[(int64_t)(h0 + h) * p.lse_head_stride + row0 + r] = d_smem[r * p.heads_per_block + h];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// bwd_finish: dQ[row, h, :] = bf16(dQ_acc[row, h, :])
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kStreamThreads)
+bwd_finish_kernel(const float4* __restrict__ acc, uint4* __restrict__ dQ, int64_t n_vec,
+                  int vec_per_row, int64_t row_stride_v) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_vec;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const float4 a = __ldcs(acc + 2 * i), b = __ldcs(acc + 2 * i + 1);
+    uint4 o;
+    o.x = pack2(a.x, a.y);
+    o.y = pack2(a.z, a.w);
+    o.z = pack2(b.x, b.y);
+    o.w = pack2(b.z, b.w);
+    const int64_t row = i / vec_per_row, c = i % vec_per_row;
+    stg_stream(dQ + row * row_stride_v + c, o);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// row fill: zero [row][head][D] bf16 rows (up to two tensors) and set fp32 [head][row] to -inf.
+// ranges: device array of (begin, end) row pairs.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kStreamThreads)
+fill_rows_kernel(const int2* __restrict__ ranges, int n_ranges, uint4* A, uint4* B, float* lse,
+                 int vec_per_row, int64_t row_stride_v, int n_heads, int64_t lse_head_stride) {
+  for (int g = blockIdx.y; g < n_ranges; g += gridDim.y) {
+    const int2 rg = ranges[g];
+    const int64_t n = (int64_t)(rg.y - rg.x) * vec_per_row;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+      const int64_t off = (rg.x + i / vec_per_row) * row_stride_v + i % vec_per_row;
+      if (A) A[off] = make_uint4(0, 0, 0, 0);
+      if (B) B[off] = make_uint4(0, 0, 0, 0);
+    }
+    if (lse) {
+      const int64_t m = (int64_t)(rg.y - rg.x) * n_heads;
+      for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m;
+           i += (int64_t)gridDim.x * blockDim.x)
+        lse[(i / (rg.y - rg.x)) * lse_head_stride + rg.x + i % (rg.y - rg.x)] = -CUDART_INF_F;
+    }
+  }
+}
+
+int pick_heads_per_block(int n_heads, int floats_per_row_head, int smem_budget_bytes) {
+  int hb = n_heads;
+  while (hb > 1 && (size_t)hb * kRowsPerTile * floats_per_row_head * 4 > (size_t)smem_budget_bytes)
+    hb = (hb + 1) / 2;
+  return hb;
+}
+
+}  // namespace
+
+namespace bs {
+
+bs_status_t validate_shape(const bs_attn_shape_t* s, const char* who) {
+  BS_REQUIRE(s != nullptr, BS_ERR_INVALID_ARG, "%s: shape is null", who);
+  BS_REQUIRE(s->head_dim == 64 || s->head_dim == 128, BS_ERR_UNSUPPORTED,
+             "%s: head_dim %d not in {64,128}", who, s->head_dim);
+  BS_REQUIRE(s->n_q_heads >= 1 && s->n_kv_heads >= 1 && s->n_q_heads % s->n_kv_heads == 0,
+             BS_ERR_INVALID_ARG, "%s: n_q_heads %d / n_kv_heads %d", who, s->n_q_heads,
+             s->n_kv_heads);
+  BS_REQUIRE(s->q_rows >= 0 && s->kv_rows >= 0, BS_ERR_INVALID_ARG, "%s: negative row count", who);
+  BS_REQUIRE(s->q_row_stride >= (int64_t)s->n_q_heads * s->head_dim && s->q_row_stride % 8 == 0,
+             BS_ERR_INVALID_ARG, "%s: q_row_stride %lld", who, (long long)s->q_row_stride);
+  BS_REQUIRE(s->kv_row_stride >= (int64_t)s->n_kv_heads * s->head_dim && s->kv_row_stride % 8 == 0,
+             BS_ERR_INVALID_ARG, "%s: kv_row_stride %lld", who, (long long)s->kv_row_stride);
+  BS_REQUIRE(s->lse_head_stride >= s->q_rows, BS_ERR_INVALID_ARG, "%s: lse_head_stride %lld < q_rows",
+             who, (long long)s->lse_head_stride);
+  return BS_OK;
+}
+
+bs_status_t launch_fill_rows(const int2* d_ranges, int n_ranges, int64_t max_rows, void* A, void* B,
+                             float* lse, int n_heads, int head_dim, int64_t row_stride,
+                             int64_t lse_head_stride, cudaStream_t st) {
+  if (n_ranges == 0) return BS_OK;
+  const int vec_per_row = n_heads * head_dim / 8;
+  int64_t bx = (max_rows * vec_per_row + kStreamThreads - 1) / kStreamThreads;
+  if (bx < 1) bx = 1;
+  if (bx > 1184) bx = 1184;
+  dim3 grid((unsigned)bx, (unsigned)(n_ranges < 64 ? n_ranges : 64));
+  fill_rows_kernel<<<grid, kStreamThreads, 0, st>>>(d_ranges, n_ranges, (uint4*)A, (uint4*)B, lse,
+                                                   vec_per_row, row_stride / 8, n_heads,
+                                                   lse_head_stride);
+  BS_CUDA(cudaGetLastError());
+  count_launch();
+  return BS_OK;
+}
+
+}  // namespace bs
+
+extern "C" {
+
+bs_status_t bs_lse_merge(int32_t n_parts, const void* const* O_parts, const float* const* LSE_parts,
+                         const bs_attn_shape_t* shape, int32_t row_begin, int32_t row_end,
+                         void* O_out, float* LSE_out, void* stream) {
+  bs_status_t rc = bs::validate_shape(shape, "bs_lse_merge");
+  if (rc != BS_OK) return rc;
+  BS_REQUIRE(n_parts >= 1 && n_parts <= BS_MAX_MERGE_PARTS, BS_ERR_INVALID_ARG,
+             "bs_lse_merge: n_parts %d outside [1,%d]", n_parts, BS_MAX_MERGE_PARTS);
+  BS_REQUIRE(O_parts && LSE_parts && O_out && LSE_out, BS_ERR_INVALID_ARG,
+             "bs_lse_merge: null pointer");
+  BS_REQUIRE(0 <= row_begin && row_begin <= row_end && row_end <= shape->q_rows, BS_ERR_INVALID_ARG,
+             "bs_lse_merge: rows [%d,%d) outside [0,%d)", row_begin, row_end, shape->q_rows);
+  MergeParams p;
+  for (int s = 0; s < n_parts; ++s) {
+    BS_REQUIRE(O_parts[s] && LSE_parts[s], BS_ERR_INVALID_ARG, "bs_lse_merge: part %d is null", s);
+    BS_REQUIRE(((uintptr_t)O_parts[s] & 15) == 0, BS_ERR_INVALID_ARG,
+               "bs_lse_merge: O_parts[%d] not 16-byte aligned", s);
+    p.O_parts[s] = (const uint4*)O_parts[s];
+    p.LSE_parts[s] = LSE_parts[s];
+  }
+  BS_REQUIRE(((uintptr_t)O_out & 15) == 0, BS_ERR_INVALID_ARG, "bs_lse_merge: O_out misaligned");
+  if (row_end == row_begin) return BS_OK;
+  p.O_out = (uint4*)O_out;
+  p.LSE_out = LSE_out;
+  p.n_parts = n_parts;
+  p.n_heads = shape->n_q_heads;
+  p.row_begin = row_begin;
+  p.row_end = row_end;
+  p.row_stride_v = shape->q_row_stride / 8;
+  p.lse_head_stride = shape->lse_head_stride;
+  p.heads_per_block = pick_heads_per_block(shape->n_q_heads, n_parts, 40 * 1024);
+  const size_t smem = (size_t)n_parts * kRowsPerTile * p.heads_per_block * sizeof(float);
+  dim3 grid((row_end - row_begin + kRowsPerTile - 1) / kRowsPerTile,
+            (shape->n_q_heads + p.heads_per_block - 1) / p.heads_per_block);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (shape->head_dim == 128)
+    lse_merge_kernel<16><<<grid, kStreamThreads, smem, st>>>(p);
+  else
+    lse_merge_kernel<8><<<grid, kStreamThreads, smem, st>>>(p);
+  BS_CUDA(cudaGetLastError());
+  bs::count_launch();
+  return BS_OK;
+}
+
+bs_status_t bs_attn_bwd_prep(const bs_attn_shape_t* shape, const void* O_final, const void* dO,
+                             float* delta, float* dQ_acc, void* stream) {
+  bs_status_t rc = bs::validate_shape(shape, "bs_attn_bwd_prep");
+  if (rc != BS_OK) return rc;
+  BS_REQUIRE(O_final && dO && delta && dQ_acc, BS_ERR_INVALID_ARG, "bs_attn_bwd_prep: null pointer");
+  BS_REQUIRE((((uintptr_t)O_final | (uintptr_t)dO | (uintptr_t)dQ_acc) & 15) == 0,
+             BS_ERR_INVALID_ARG, "bs_attn_bwd_prep: pointers must be 16-byte aligned");
+  if (shape->q_rows == 0) return BS_OK;
+  PrepParams p;
+  p.O = (const uint4*)O_final;
+  p.dO = (const uint4*)dO;
+  p.delta = delta;
+  p.dQ_acc = (float4*)dQ_acc;
+  p.n_heads = shape->n_q_heads;
+  p.rows = shape->q_rows;
+  p.row_stride_v = shape->q_row_stride / 8;
+  p.lse_head_stride = shape->lse_head_stride;
+  p.heads_per_block = pick_heads_per_block(shape->n_q_heads, 1, 16 * 1024);
+  if (p.heads_per_block > 32) p.heads_per_block = 32;  // keep enough blocks in flight
+  const size_t smem = (size_t)kRowsPerTile * p.heads_per_block * sizeof(float);
+  dim3 grid((shape->q_rows + kRowsPerTile - 1) / kRowsPerTile,
+            (shape->n_q_heads + p.heads_per_block - 1) / p.heads_per_block);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (shape->head_dim == 128)
+    bwd_prep_kernel<16><<<grid, kStreamThreads, smem, st>>>(p);
+  else
+    bwd_prep_kernel<8><<<grid, kStreamThreads, smem, st>>>(p);
+  BS_CUDA(cudaGetLastError());
+  bs::count_launch();
+  return BS_OK;
+}
+
+bs_status_t bs_attn_bwd_finish(const bs_attn_shape_t* shape, const float* dQ_acc, void* dQ,
+                               void* stream) {
+  bs_status_t rc = bs::validate_shape(shape, "bs_attn_bwd_finish");
+  if (rc != BS_OK) return rc;
+  BS_REQUIRE(dQ_acc && dQ, BS_ERR_INVALID_ARG, "bs_attn_bwd_finish: null pointer");
+  BS_REQUIRE((((uintptr_t)dQ_acc | (uintptr_t)dQ) & 15) == 0, BS_ERR_INVALID_ARG,
+             "bs_attn_bwd_finish: pointers must be 16-byte aligned");
+  if (shape->q_rows == 0) return BS_OK;
+  const int vec_per_row = shape->n_q_heads * shape->head_dim / 8;
+  const int64_t n_vec = (int64_t)shape->q_rows * vec_per_row;
+  int64_t blocks = (n_vec + kStreamThreads - 1) / kStreamThreads;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  bwd_finish_kernel<<<(unsigned)blocks, kStreamThreads, 0, (cudaStream_t)stream>>>(
+      (const float4*)dQ_acc, (uint4*)dQ, n_vec, vec_per_row, shape->q_row_stride / 8);
+  BS_CUDA(cudaGetLastError());
+  bs::count_launch();
+  return BS_OK;
+}
+
+}  // extern "C"

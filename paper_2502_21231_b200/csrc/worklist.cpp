@@ -1,0 +1,180 @@
+// worklist.cpp — host builder of the attention work-item tables (see worklist.h).
+#include "worklist.h"
+
+#include <algorithm>
+#include <new>
+
+namespace bs {
+
+namespace {
+inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
+inline int32_t ceil_div(int64_t a, int64_t b) { return (int32_t)((a + b - 1) / b); }
+
+struct Range {
+  int32_t begin, end;
+  bool operator<(const Range& o) const { return begin < o.begin; }
+};
+
+// Check that ranges (sorted by begin, duplicates removed) are pairwise disjoint and list the gaps
+// of [lo,hi) they leave uncovered.
+bs_status_t gaps_of(const std::vector<Range>& rs, int32_t lo, int32_t hi, const char* what,
+                    SchedTables* out) {
+  int32_t cur = lo;
+  for (const Range& r : rs) {
+    BS_REQUIRE(r.begin >= cur || r.begin == lo, BS_ERR_INVALID_ARG,
+               "%s ranges of two segments overlap without being identical (at row %d)", what,
+               r.begin);
+    BS_REQUIRE(r.begin >= cur, BS_ERR_INVALID_ARG,
+               "%s ranges of two segments overlap without being identical (at row %d)", what,
+               r.begin);
+    if (r.begin > cur) out->fill.push_back({cur, r.begin});
+    cur = r.end;
+  }
+  if (cur < hi) out->fill.push_back({cur, hi});
+  out->max_fill_rows = 0;
+  for (const RowRange& f : out->fill)
+    out->max_fill_rows = std::max<int64_t>(out->max_fill_rows, f.end - f.begin);
+  return BS_OK;
+}
+
+bs_status_t check_seg(const bs_seg_t& g, int i, int32_t q_rows, int32_t kv_rows) {
+  BS_REQUIRE(0 <= g.q_begin && g.q_begin < g.q_end && g.q_end <= q_rows, BS_ERR_INVALID_ARG,
+             "segment %d: q range [%d,%d) empty or outside [0,%d)", i, g.q_begin, g.q_end, q_rows);
+  BS_REQUIRE(0 <= g.k_begin && g.k_begin < g.k_end && g.k_end <= kv_rows, BS_ERR_INVALID_ARG,
+             "segment %d: k range [%d,%d) empty or outside [0,%d)", i, g.k_begin, g.k_end, kv_rows);
+  return BS_OK;
+}
+}  // namespace
+
+WsLayout ws_layout(size_t n_items, size_t n_spans, size_t n_fill) {
+  WsLayout L;
+  L.items_off = sizeof(SchedHeader);
+  L.spans_off = align256(L.items_off + n_items * sizeof(Item));
+  L.fill_off = align256(L.spans_off + n_spans * sizeof(Span));
+  L.total = align256(L.fill_off + n_fill * sizeof(RowRange));
+  return L;
+}
+
+size_t ws_upper_bound(int64_t rows, int32_t n_segs, bool bwd) {
+  // items: every distinct range of length L yields ceil(L / tile) <= L / tile + 1 items
+  const int64_t tile = bwd ? kTile : 2 * kTile;
+  const size_t n_items = (size_t)(rows / tile + n_segs + 1);
+  return ws_layout(n_items, (size_t)n_segs, (size_t)n_segs + 1).total;
+}
+
+bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_rows, int32_t kv_rows,
+                             int32_t out_begin, int32_t out_end, SchedTables* out) {
+  try {
+    std::vector<int32_t> order(n_segs);
+    for (int32_t i = 0; i < n_segs; ++i) {
+      bs_status_t rc = check_seg(segs[i], i, q_rows, kv_rows);
+      if (rc != BS_OK) return rc;
+      BS_REQUIRE(segs[i].q_begin >= out_begin && segs[i].q_end <= out_end, BS_ERR_INVALID_ARG,
+                 "segment %d: q range [%d,%d) outside the output rows [%d,%d)", i, segs[i].q_begin,
+                 segs[i].q_end, out_begin, out_end);
+      order[i] = i;
+    }
+    // group by q range; keep the caller's order inside a group
+    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) {
+      return segs[a].q_begin != segs[b].q_begin ? segs[a].q_begin < segs[b].q_begin
+                                                : segs[a].q_end < segs[b].q_end;
+    });
+    std::vector<Range> ranges;
+    for (int32_t i = 0; i < n_segs;) {
+      const bs_seg_t& g0 = segs[order[i]];
+      int32_t j = i;
+      const int32_t span_begin = (int32_t)out->spans.size();
+      while (j < n_segs && segs[order[j]].q_begin == g0.q_begin &&
+             segs[order[j]].q_end == g0.q_end) {
+        const bs_seg_t& g = segs[order[j]];
+        out->spans.push_back({g.k_begin, g.k_end - g.k_begin, g.causal_offset, 0});
+        ++j;
+      }
+      ranges.push_back({g0.q_begin, g0.q_end});
+      const int32_t q_len = g0.q_end - g0.q_begin;
+      for (int32_t a0 = 0; a0 < q_len; a0 += 2 * kTile) {
+        Item it{};
+        it.row0 = g0.q_begin + a0;
+        it.local0 = a0;
+        it.range_len = q_len;
+        it.span_begin = span_begin;
+        it.n_spans = j - i;
+        int32_t cost = 0;
+        for (int t = 0; t < 2; ++t) {
+          const int32_t at = a0 + t * kTile;
+          if (at >= q_len) break;
+          const int64_t a_last = std::min<int64_t>(at + kTile, q_len) - 1;
+          for (int32_t s = span_begin; s < span_begin + it.n_spans; ++s) {
+            const int64_t vis = std::min<int64_t>(out->spans[s].len, a_last + out->spans[s].off + 1);
+            if (vis > 0) cost += ceil_div(vis, kTile);
+          }
+        }
+        it.cost = cost;
+        out->items.push_back(it);
+      }
+      i = j;
+    }
+    std::stable_sort(out->items.begin(), out->items.end(),
+                     [](const Item& a, const Item& b) { return a.cost > b.cost; });
+    std::sort(ranges.begin(), ranges.end());
+    return gaps_of(ranges, out_begin, out_end, "query", out);
+  } catch (const std::bad_alloc&) {
+    return fail(BS_ERR_HOST_OOM, "out of host memory building the forward work list");
+  }
+}
+
+bs_status_t build_bwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_rows, int32_t kv_rows,
+                             SchedTables* out) {
+  try {
+    std::vector<int32_t> order(n_segs);
+    for (int32_t i = 0; i < n_segs; ++i) {
+      bs_status_t rc = check_seg(segs[i], i, q_rows, kv_rows);
+      if (rc != BS_OK) return rc;
+      order[i] = i;
+    }
+    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) {
+      return segs[a].k_begin != segs[b].k_begin ? segs[a].k_begin < segs[b].k_begin
+                                                : segs[a].k_end < segs[b].k_end;
+    });
+    std::vector<Range> ranges;
+    for (int32_t i = 0; i < n_segs;) {
+      const bs_seg_t& g0 = segs[order[i]];
+      int32_t j = i;
+      const int32_t span_begin = (int32_t)out->spans.size();
+      while (j < n_segs && segs[order[j]].k_begin == g0.k_begin &&
+             segs[order[j]].k_end == g0.k_end) {
+        const bs_seg_t& g = segs[order[j]];
+        out->spans.push_back({g.q_begin, g.q_end - g.q_begin, g.causal_offset, 0});
+        ++j;
+      }
+      ranges.push_back({g0.k_begin, g0.k_end});
+      const int32_t k_len = g0.k_end - g0.k_begin;
+      for (int32_t b0 = 0; b0 < k_len; b0 += kTile) {
+        Item it{};
+        it.row0 = g0.k_begin + b0;
+        it.local0 = b0;
+        it.range_len = k_len;
+        it.span_begin = span_begin;
+        it.n_spans = j - i;
+        int32_t cost = 0;
+        for (int32_t s = span_begin; s < span_begin + it.n_spans; ++s) {
+          // query a sees key b0 iff a >= b0 - off: query tiles from floor(a_min / tile) on
+          const int64_t a_min = std::max<int64_t>(0, (int64_t)b0 - out->spans[s].off);
+          if (a_min < out->spans[s].len)
+            cost += ceil_div(out->spans[s].len, kTile) - (int32_t)(a_min / kTile);
+        }
+        it.cost = cost;
+        out->items.push_back(it);
+      }
+      i = j;
+    }
+    std::stable_sort(out->items.begin(), out->items.end(),
+                     [](const Item& a, const Item& b) { return a.cost > b.cost; });
+    std::sort(ranges.begin(), ranges.end());
+    return gaps_of(ranges, 0, kv_rows, "key", out);
+  } catch (const std::bad_alloc&) {
+    return fail(BS_ERR_HOST_OOM, "out of host memory building the backward work list");
+  }
+}
+
+}  // namespace bs

@@ -1,0 +1,70 @@
+// worklist.h — work-item tables of the attention kernels (host-built, uploaded into the caller's
+// workspace).  This is the single-device analogue of the paper's balance scheduler (Alg. 2,
+// sort by cost descending, keep every worker equally loaded): items are ordered
+// longest-first and pulled by persistent CTAs.
+//
+// Forward item  = up to 256 consecutive query rows (two 128-row MMA tiles) of one distinct query
+//                 range; its spans are the key ranges of every segment on that query range
+//                 (softmax over the union).  The kernel multiplies the item list by the Q heads.
+// Backward item = one 128-key tile of one distinct key range; its spans are the query ranges of
+//                 every segment on that key range.  The kernel multiplies the list by the KV heads
+//                 and loops over the G query heads of the group and the visible query tiles.
+#pragma once
+#include <cstdint>
+#include <vector>
+
+#include "common.h"
+
+namespace bs {
+
+constexpr int kTile = 128;  // MMA tile edge in rows / keys
+
+struct Span {     // forward: a key range;  backward: a query range
+  int32_t begin;  // first row in the K/V (fwd) or Q (bwd) buffer
+  int32_t len;    // rows
+  int32_t off;    // key b visible to query a  iff  b <= a + off  (a, b local to their ranges)
+  int32_t pad;
+};
+struct Item {
+  int32_t row0;        // first buffer row of the item (fwd: Q rows; bwd: K/V rows)
+  int32_t local0;      // index of row0 inside its range (fwd: a0; bwd: b0)
+  int32_t range_len;   // length of the range the item belongs to (q_len fwd, k_len bwd)
+  int32_t span_begin;  // first span in the span table
+  int32_t n_spans;
+  int32_t cost;        // 128x128 blocks the item visits per head
+  int32_t pad[2];
+};
+struct RowRange {
+  int32_t begin, end;
+};
+struct SchedHeader {  // first 256 bytes of the workspace
+  int32_t counter;    // dynamic scheduler cursor (zeroed by the upload)
+  int32_t n_items, n_spans, n_fill;
+  int32_t pad[60];
+};
+static_assert(sizeof(SchedHeader) == 256, "header size");
+static_assert(sizeof(Item) == 32 && sizeof(Span) == 16, "table element sizes");
+
+struct SchedTables {
+  std::vector<Item> items;     // sorted by cost, descending
+  std::vector<Span> spans;
+  std::vector<RowRange> fill;  // rows of the output range covered by no item
+  int64_t max_fill_rows = 0;
+};
+
+// Workspace layout: [SchedHeader][items][spans][fill ranges], each 256-byte aligned.
+struct WsLayout {
+  size_t items_off, spans_off, fill_off, total;
+};
+WsLayout ws_layout(size_t n_items, size_t n_spans, size_t n_fill);
+// Upper bounds used by bs_attn_workspace_bytes (no segment list yet).
+size_t ws_upper_bound(int64_t rows, int32_t n_segs, bool bwd);
+
+// Forward: group segments by query range; rows [out_begin,out_end) not covered go to `fill`.
+bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_rows, int32_t kv_rows,
+                             int32_t out_begin, int32_t out_end, SchedTables* out);
+// Backward: group segments by key range; all kv_rows rows not covered go to `fill`.
+bs_status_t build_bwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_rows, int32_t kv_rows,
+                             SchedTables* out);
+
+}  // namespace bs
