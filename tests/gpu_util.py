@@ -1,0 +1,160 @@
+"""Helpers of the -m gpu parity tests: build a workload's tensors once (seeded generator), run
+the CUDA path through the C-ABI binding, run the oracle on the same inputs, compare."""
+import numpy as np
+import torch
+
+import oracle
+from paper_2502_21231_b200 import binding as B
+from paper_2502_21231_b200.synth import rng, workloads
+
+# BASELINE.json north_star tolerances
+TOL_O = 1.5e-2      # max abs
+TOL_LSE = 1e-3      # abs
+TOL_GRAD = 1e-2     # relative L2
+
+
+def to_dev(bits):
+    """uint16 bf16 bit patterns (numpy) -> torch.bfloat16 CUDA tensor."""
+    return torch.from_numpy(bits.view(np.int16)).cuda().view(torch.bfloat16)
+
+
+def to_bits(t):
+    return t.detach().view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+def rel_l2(got, want):
+    want = np.asarray(want, np.float64)
+    got = np.asarray(got, np.float64)
+    den = np.sqrt((want ** 2).sum())
+    return float(np.sqrt(((got - want) ** 2).sum()) / den) if den > 0 else float(np.abs(got).max())
+
+
+class DeviceRun:
+    """One simulated rank: local Q/dO, per-step K/V, plan from the LIBRARY (bs_plan)."""
+
+    def __init__(self, w, steps=None, gen_kv=True):
+        self.w = w
+        self.plan = B.plan(w.seqs)
+        self.Hq, self.Hkv, self.D = w.n_q_heads, w.n_kv_heads, w.head_dim
+        pl = self.plan
+        self.q_rows = pl["q_rows"]
+        qruns = workloads.runs_from(pl["q_seq"], pl["q_pos"])
+        self.Q_bits = workloads.gen_rows(w.seed, rng.STREAM_Q, qruns, self.Hq * self.D)
+        self.dO_bits = workloads.gen_rows(w.seed, rng.STREAM_DO, qruns, self.Hq * self.D)
+        self.steps = list(range(pl["n_steps"])) if steps is None else steps
+        self.K_bits, self.V_bits = {}, {}
+        if gen_kv:
+            for s in self.steps:
+                st = pl["steps"][s]
+                kruns = workloads.runs_from(st["k_seq"], st["k_pos"])
+                self.K_bits[s] = workloads.gen_rows(w.seed, rng.STREAM_K, kruns, self.Hkv * self.D)
+                self.V_bits[s] = workloads.gen_rows(w.seed, rng.STREAM_V, kruns, self.Hkv * self.D)
+
+    def shape(self, step):
+        return B.make_shape(self.Hq, self.Hkv, self.D, self.q_rows,
+                            self.plan["steps"][step]["kv_rows"])
+
+    def q3(self, bits):
+        return bits.reshape(-1, self.Hq, self.D)
+
+    def kv3(self, bits):
+        return bits.reshape(-1, self.Hkv, self.D)
+
+    def forward(self, merge=True):
+        """Run every step's bs_attn_fwd and (if more than one step) bs_lse_merge.
+        Returns (O bf16 cuda [q_rows,Hq,D], LSE f32 cuda [Hq,q_rows], per-step partials)."""
+        Q = to_dev(self.Q_bits)
+        parts = []
+        for s in self.steps:
+            st = self.plan["steps"][s]
+            sh = self.shape(s)
+            K, V = to_dev(self.K_bits[s]), to_dev(self.V_bits[s])
+            O = torch.full((self.q_rows, self.Hq, self.D), float("nan"), dtype=torch.bfloat16,
+                           device="cuda")
+            LSE = torch.full((self.Hq, self.q_rows), float("nan"), dtype=torch.float32,
+                             device="cuda")
+            ws = torch.empty(B.attn_workspace_bytes(sh, len(st["segs"]), False), dtype=torch.uint8,
+                             device="cuda")
+            B.attn_fwd(sh, Q, K, V, st["segs"], (0, self.q_rows), O, LSE, ws)
+            parts.append((O, LSE))
+        torch.cuda.synchronize()
+        if len(parts) == 1 or not merge:
+            return parts[0][0], parts[0][1], parts
+        O = torch.empty_like(parts[0][0])
+        LSE = torch.empty_like(parts[0][1])
+        B.lse_merge([p[0] for p in parts], [p[1] for p in parts], self.shape(self.steps[0]),
+                    (0, self.q_rows), O, LSE)
+        torch.cuda.synchronize()
+        return O, LSE, parts
+
+    def backward(self, O, LSE):
+        """prep, every step's bs_attn_bwd, finish.  Returns dQ bf16, {step: (dK, dV)}."""
+        Q, dO = to_dev(self.Q_bits), to_dev(self.dO_bits)
+        sh0 = self.shape(self.steps[0])
+        delta = torch.empty((self.Hq, self.q_rows), dtype=torch.float32, device="cuda")
+        dQ_acc = torch.full((self.q_rows, self.Hq, self.D), float("nan"), dtype=torch.float32,
+                            device="cuda")
+        B.attn_bwd_prep(sh0, O, dO, delta, dQ_acc)
+        grads = {}
+        for s in self.steps:
+            st = self.plan["steps"][s]
+            sh = self.shape(s)
+            K, V = to_dev(self.K_bits[s]), to_dev(self.V_bits[s])
+            dK = torch.full_like(K.view(-1, self.Hkv, self.D), float("nan"))
+            dV = torch.full_like(dK, float("nan"))
+            ws = torch.empty(B.attn_workspace_bytes(sh, len(st["segs"]), True), dtype=torch.uint8,
+                             device="cuda")
+            B.attn_bwd(sh, Q, K, V, dO, LSE, delta, st["segs"], dQ_acc, dK, dV, ws)
+            grads[s] = (dK, dV)
+        dQ = torch.empty((self.q_rows, self.Hq, self.D), dtype=torch.bfloat16, device="cuda")
+        B.attn_bwd_finish(sh0, dQ_acc, dQ)
+        torch.cuda.synchronize()
+        return dQ, grads, delta
+
+    # ------------------------------------------------------------------ oracle side
+    def oracle_all_keys(self):
+        """(K_bits, V_bits, k_seq, k_pos) of the union of all steps' KV buffers, taken from the
+        ORACLE planner (independent of the library's plan)."""
+        opl = oracle.oracle_plan(self.w.seqs)
+        ks = np.concatenate([opl["steps"][s]["k_seq"] for s in self.steps])
+        kp = np.concatenate([opl["steps"][s]["k_pos"] for s in self.steps])
+        Kb = np.concatenate([self.K_bits[s] for s in self.steps])
+        Vb = np.concatenate([self.V_bits[s] for s in self.steps])
+        return opl, Kb, Vb, ks, kp
+
+    def oracle_forward(self, rows=None):
+        opl, Kb, Vb, ks, kp = self.oracle_all_keys()
+        qs, qp = opl["q_seq"], opl["q_pos"]
+        Qb = self.q3(self.Q_bits)
+        if rows is not None:
+            qs, qp, Qb = qs[rows], qp[rows], Qb[rows]
+        return oracle.attn_fwd(Qb, self.kv3(Kb), self.kv3(Vb), qs, qp, ks, kp)
+
+    def oracle_backward(self):
+        opl, Kb, Vb, ks, kp = self.oracle_all_keys()
+        dQ, dK, dV = oracle.attn_bwd(self.q3(self.Q_bits), self.kv3(Kb), self.kv3(Vb),
+                                     self.q3(self.dO_bits), opl["q_seq"], opl["q_pos"], ks, kp)
+        # split dK/dV back per step
+        out, row = {}, 0
+        for s in self.steps:
+            n = opl["steps"][s]["kv_rows"]
+            out[s] = (dK[row:row + n], dV[row:row + n])
+            row += n
+        return dQ, out
+
+
+def check_forward(run, O, LSE, rows=None):
+    Oo, Lo = run.oracle_forward(rows)
+    got_O = oracle.bf16_to_f64(to_bits(O)).reshape(run.q_rows, run.Hq, run.D)
+    got_L = LSE.double().cpu().numpy()
+    if rows is not None:
+        got_O, got_L = got_O[rows], got_L[:, rows]
+    assert not np.isnan(got_O).any() and not np.isnan(got_L).any()
+    err_O = float(np.abs(got_O - Oo).max())
+    fin = np.isfinite(Lo)
+    assert np.array_equal(np.isneginf(got_L), np.isneginf(Lo))
+    err_L = float(np.abs(got_L[fin] - Lo[fin]).max()) if fin.any() else 0.0
+    assert np.all(got_O[~fin.T] == 0)
+    assert err_O <= TOL_O, f"O max abs err {err_O}"
+    assert err_L <= TOL_LSE, f"LSE abs err {err_L}"
+    return err_O, err_L
