@@ -1,7 +1,572 @@
-// attn_bwd.cu — bs_attn_bwd (placeholder while the tcgen05 backward kernel is brought up).
+// attn_bwd.cu — bs_attn_bwd: backward of one Q-chunk x KV-chunk step on sm_100a (SURVEY.md 8(a)
+// a6; gradients of softmax attention as in flash-attention backward).
+//
+// One persistent CTA per SM, 384 threads:
+//   warps 0-3  compute warpgroup A: query columns  0..63  of the 128x128 tile
+//   warps 4-7  compute warpgroup B: query columns 64..127
+//   warp  8    MMA issuer (one lane)          warp 9  TMA producer (+ LSE/delta staging)
+// A work item is (one 128-key tile of a key range, one KV head).  The CTA keeps dK and dV of the
+// tile in TMEM and loops over the G query heads of the group and over every 128-row query tile
+// that sees the key tile; per iteration it issues the five MMAs of flash-attention backward, all
+// with keys on the TMEM lanes ("transposed" form, thread r <-> key row r):
+//   S^T  = K Q^T                  (SS)   -> P^T = exp2(S^T c - LSE)        written back to TMEM
+//   dP^T = V dO^T                 (SS)   -> dS^T = P^T * (dP^T - delta) c  written to smem (bf16)
+//   dV  += P^T dO                 (TS, A = P^T from TMEM, B = dO MN-major)
+//   dK  += dS^T Q                 (SS, A = dS^T K-major, B = Q MN-major)
+//   dQ   = dS K                   (SS, A = dS^T read MN-major, B = K MN-major) -> TMEM -> smem
+//                                  -> TMA reduce-add (fp32) into dQ_acc
+// TMEM: [0,128) S^T / P^T   [128,256) dP^T, then dQ   [256,256+D) dK   [384,384+D) dV.
+// dK/dV are therefore reduced over the group's heads inside the kernel (no atomics); dQ is
+// reduced across key tiles and steps by the TMA unit in L2.
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <math_constants.h>
+
 #include "common.h"
-extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t*, const void*, const void*, const void*,
-                                   const void*, const float*, const float*, const bs_seg_t*,
-                                   int32_t, float*, void*, void*, void*, size_t, void*) {
-  return bs::fail(BS_ERR_UNSUPPORTED, "bs_attn_bwd: not built yet");
+#include "launch_utils.h"
+#include "ptx.cuh"
+#include "worklist.h"
+
+namespace {
+
+using namespace bs;
+using namespace bs::ptx;
+
+constexpr int kBwdThreads = 384;
+constexpr int kComputeThreads = 256;
+
+struct BwdParams {
+  const Item* items;
+  const Span* spans;
+  int32_t n_items;  // key-tile items (x n_kv_heads work items)
+  int32_t n_kv_heads, group;
+  int32_t q_rows;
+  float scale, scale_log2;
+  const float* LSE;
+  const float* delta;
+  int64_t lse_head_stride;
+  __nv_bfloat16* dK;
+  __nv_bfloat16* dV;
+  int64_t kv_row_stride;
+};
+
+template <int D>
+struct BwdSmem {
+  static constexpr int kTileBytes = kTile * D * 2;      // K, V, Q, dO tiles
+  static constexpr int kKOff = 0;
+  static constexpr int kVOff = kTileBytes;
+  static constexpr int kQOff = 2 * kTileBytes;          // 2 stages
+  static constexpr int kDOOff = 4 * kTileBytes;         // 1 stage
+  static constexpr int kDSOff = 5 * kTileBytes;         // dS^T [128 keys][128 queries] bf16
+  static constexpr int kDQOff = kDSOff + kTile * kTile * 2;  // 2 x [128][32] fp32 staging
+  static constexpr int kLseOff = kDQOff + 2 * kTile * 128;   // [2 stages][128] lse*log2e
+  static constexpr int kDeltaOff = kLseOff + 2 * kTile * 4;  // [2 stages][128] delta*scale
+  static constexpr int kBarOff = kDeltaOff + 2 * kTile * 4;
+  // kv_full kv_empty q_full[2] q_empty[2] do_full do_empty s_full p_full dp_full ds_full dq_full
+  // dq_drained acc_full acc_empty
+  static constexpr int kNumBars = 16;
+  static constexpr int kTmemSlotOff = kBarOff + kNumBars * 8;
+  static constexpr int kBytes = kTmemSlotOff + 16;
+};
+
+// Iterations of one item: for each query head of the group, for each span (query range), the
+// 128-row query tiles holding at least one query that sees the key tile's first key.
+struct BwdWalker {
+  const Span* spans;
+  int n_spans, group, b0, hi, s, qi, n_qt;
+  Span sp;
+  __device__ __forceinline__ void load_span() {
+    while (hi < group) {
+      while (s < n_spans) {
+        sp = spans[s];
+        const int a_min = max(0, b0 - sp.off);  // first query that sees key b0
+        if (a_min < sp.len) {
+          qi = a_min / kTile;
+          n_qt = (sp.len + kTile - 1) / kTile;
+          return;
+        }
+        ++s;
+      }
+      ++hi;
+      s = 0;
+    }
+  }
+  __device__ __forceinline__ void init(const Span* table, const Item& it, int g) {
+    spans = table + it.span_begin;
+    n_spans = it.n_spans;
+    group = g;
+    b0 = it.local0;
+    hi = 0;
+    s = 0;
+    load_span();
+  }
+  __device__ __forceinline__ bool done() const { return hi >= group; }
+  __device__ __forceinline__ void next() {
+    if (++qi >= n_qt) {
+      ++s;
+      load_span();
+    }
+  }
+  __device__ __forceinline__ int q_row() const { return sp.begin + qi * kTile; }
+};
+
+// SS MMA, both operands K-major 128-row tiles (S^T = K Q^T, dP^T = V dO^T)
+template <int D>
+__device__ __forceinline__ void issue_kmajor(uint32_t tmem_d, uint32_t a_addr, uint32_t b_addr) {
+  constexpr uint32_t idesc = umma_idesc_bf16(kTile, kTile, 0, 0);
+#pragma unroll
+  for (int kk = 0; kk < D / 16; ++kk) {
+    const uint32_t o = (kk / 4) * (kTile * 128) + (kk % 4) * 32;
+    umma_ss(tmem_d, umma_desc_sw128(a_addr + o, 16, 1024), umma_desc_sw128(b_addr + o, 16, 1024),
+            idesc, kk > 0);
+  }
+}
+// dV += P^T dO : A from TMEM (packed bf16), B = dO [queries][D] MN-major
+template <int D>
+__device__ __forceinline__ void issue_dv(uint32_t tmem_d, uint32_t tmem_p, uint32_t do_addr,
+                                         bool accumulate) {
+  constexpr uint32_t idesc = umma_idesc_bf16(kTile, D, 0, 1);
+#pragma unroll
+  for (int kk = 0; kk < kTile / 16; ++kk)
+    umma_ts(tmem_d, tmem_p + (kk / 4) * 64 + (kk % 4) * 8,  // P^T halves at columns [0,32), [64,96)
+            umma_desc_sw128(do_addr + kk * 2048, kTile * 128, 1024), idesc, accumulate || kk > 0);
+}
+// dK += dS^T Q : A = dS^T [keys][queries] K-major (two 64-query boxes), B = Q MN-major
+template <int D>
+__device__ __forceinline__ void issue_dk(uint32_t tmem_d, uint32_t ds_addr, uint32_t q_addr,
+                                         bool accumulate) {
+  constexpr uint32_t idesc = umma_idesc_bf16(kTile, D, 0, 1);
+#pragma unroll
+  for (int kk = 0; kk < kTile / 16; ++kk) {
+    const uint32_t o = (kk / 4) * (kTile * 128) + (kk % 4) * 32;
+    umma_ss(tmem_d, umma_desc_sw128(ds_addr + o, 16, 1024),
+            umma_desc_sw128(q_addr + kk * 2048, kTile * 128, 1024), idesc, accumulate || kk > 0);
+  }
+}
+// dQ = dS K : A = the same dS^T smem read MN-major (M = queries contiguous), B = K MN-major
+template <int D>
+__device__ __forceinline__ void issue_dq(uint32_t tmem_d, uint32_t ds_addr, uint32_t k_addr) {
+  constexpr uint32_t idesc = umma_idesc_bf16(kTile, D, 1, 1);
+#pragma unroll
+  for (int kk = 0; kk < kTile / 16; ++kk)
+    umma_ss(tmem_d, umma_desc_sw128(ds_addr + kk * 2048, kTile * 128, 1024),
+            umma_desc_sw128(k_addr + kk * 2048, kTile * 128, 1024), idesc, kk > 0);
+}
+
+}  // namespace
+
+namespace {
+
+template <int D>
+__global__ void __launch_bounds__(kBwdThreads, 1)
+attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmDO,
+                const __grid_constant__ CUtensorMap tmDQ, const __grid_constant__ BwdParams p) {
+  using L = BwdSmem<D>;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::kBarOff);
+  uint64_t* kv_full = bars + 0;
+  uint64_t* kv_empty = bars + 1;
+  uint64_t* q_full = bars + 2;   // [2]
+  uint64_t* q_empty = bars + 4;  // [2]
+  uint64_t* do_full = bars + 6;
+  uint64_t* do_empty = bars + 7;
+  uint64_t* s_full = bars + 8;
+  uint64_t* p_full = bars + 9;
+  uint64_t* dp_full = bars + 10;
+  uint64_t* ds_full = bars + 11;
+  uint64_t* dq_full = bars + 12;
+  uint64_t* dq_drained = bars + 13;
+  uint64_t* acc_full = bars + 14;
+  uint64_t* acc_empty = bars + 15;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kTmemSlotOff);
+  float* lse_s = reinterpret_cast<float*>(smem + L::kLseOff);
+  float* delta_s = reinterpret_cast<float*>(smem + L::kDeltaOff);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0 && (smem_u32(smem) & 1023u) != 0) {
+    printf("bs_attn_bwd: dynamic shared memory base is not 1024-byte aligned\n");
+    __trap();
+  }
+  if (warp == 9 && lane == 0) {
+    mbar_init(kv_full, 1);
+    mbar_init(kv_empty, 1);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(&q_full[i], 33);  // expect_tx arrive + 32 lanes staging LSE/delta
+      mbar_init(&q_empty[i], 1);
+    }
+    mbar_init(do_full, 1);
+    mbar_init(do_empty, 1);
+    mbar_init(s_full, 1);
+    mbar_init(p_full, kComputeThreads);
+    mbar_init(dp_full, 1);
+    mbar_init(ds_full, kComputeThreads);
+    mbar_init(dq_full, 1);
+    mbar_init(dq_drained, kComputeThreads);
+    mbar_init(acc_full, 1);
+    mbar_init(acc_empty, kComputeThreads);
+    fence_barrier_init();
+    prefetch_tensormap(&tmQ);
+    prefetch_tensormap(&tmK);
+    prefetch_tensormap(&tmV);
+    prefetch_tensormap(&tmDO);
+    prefetch_tensormap(&tmDQ);
+  }
+  if (warp == 8) tmem_alloc<512>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *tmem_slot;
+  const uint32_t sK = smem_u32(smem + L::kKOff), sV = smem_u32(smem + L::kVOff);
+  const uint32_t sQ = smem_u32(smem + L::kQOff), sDO = smem_u32(smem + L::kDOOff);
+  const uint32_t sDS = smem_u32(smem + L::kDSOff);
+  const int total_work = p.n_items * p.n_kv_heads;
+
+  if (warp == 9) {
+    // ============================ TMA producer + LSE/delta staging ============================
+    uint32_t item_n = 0, it_n = 0;  // items / iterations issued so far (ring phases)
+    for (int w = blockIdx.x; w < total_work; w += gridDim.x) {
+      const Item it = p.items[w / p.n_kv_heads];
+      const int g = w % p.n_kv_heads;
+      BwdWalker wk;
+      wk.init(p.spans, it, p.group);
+      if (wk.done()) continue;
+      if (lane == 0) {
+        mbar_wait(kv_empty, (item_n & 1) ^ 1);
+        mbar_arrive_expect_tx(kv_full, 2 * L::kTileBytes);
+        for (int half = 0; half < D / 64; ++half) {
+          tma_load_3d(smem + L::kKOff + half * (kTile * 128), &tmK, kv_full, half * 64, g, it.row0);
+          tma_load_3d(smem + L::kVOff + half * (kTile * 128), &tmV, kv_full, half * 64, g, it.row0);
+        }
+      }
+      ++item_n;
+      for (; !wk.done(); wk.next(), ++it_n) {
+        const int st = it_n & 1, h = g * p.group + wk.hi, qrow = wk.q_row();
+        mbar_wait(&q_empty[st], ((it_n >> 1) & 1) ^ 1);
+        if (lane == 0) {
+          mbar_arrive_expect_tx(&q_full[st], L::kTileBytes);
+          for (int half = 0; half < D / 64; ++half)
+            tma_load_3d(smem + L::kQOff + st * L::kTileBytes + half * (kTile * 128), &tmQ,
+                        &q_full[st], half * 64, h, qrow);
+        }
+        // lse*log2e (+inf for rows outside the query range: P becomes exactly 0) and delta*scale
+        for (int c = lane; c < kTile; c += 32) {
+          const int a = wk.qi * kTile + c;
+          const bool ok = a < wk.sp.len;
+          const int64_t idx = (int64_t)h * p.lse_head_stride + qrow + c;
+          lse_s[st * kTile + c] = ok ? p.LSE[idx] * 1.4426950408889634f : CUDART_INF_F;
+          delta_s[st * kTile + c] = ok ? p.delta[idx] * p.scale : 0.f;
+        }
+        mbar_arrive(&q_full[st]);
+        if (lane == 0) {
+          mbar_wait(do_empty, (it_n & 1) ^ 1);
+          mbar_arrive_expect_tx(do_full, L::kTileBytes);
+          for (int half = 0; half < D / 64; ++half)
+            tma_load_3d(smem + L::kDOOff + half * (kTile * 128), &tmDO, do_full, half * 64, h, qrow);
+        }
+        __syncwarp();
+      }
+    }
+  } else if (warp == 8) {
+    // ======================================= MMA issuer =======================================
+    if (lane == 0) {
+      uint32_t item_n = 0, it_n = 0;
+      for (int w = blockIdx.x; w < total_work; w += gridDim.x) {
+        const Item it = p.items[w / p.n_kv_heads];
+        BwdWalker wk;
+        wk.init(p.spans, it, p.group);
+        if (wk.done()) continue;
+        mbar_wait(kv_full, item_n & 1);
+        mbar_wait(acc_empty, (item_n & 1) ^ 1);  // previous item's dK/dV have left TMEM
+        tc_fence_after();
+        // prologue: S^T(0)
+        mbar_wait(&q_full[it_n & 1], (it_n >> 1) & 1);
+        tc_fence_after();
+        issue_kmajor<D>(tmem, sK, sQ + (it_n & 1) * L::kTileBytes);
+        tc_commit(s_full);
+        bool first = true;
+        while (true) {
+          BwdWalker nxt = wk;
+          nxt.next();
+          const bool has_next = !nxt.done();
+          const uint32_t st = it_n & 1;
+          // dV += P^T dO
+          mbar_wait(do_full, it_n & 1);
+          mbar_wait(p_full, it_n & 1);
+          tc_fence_after();
+          issue_dv<D>(tmem + 384, tmem, sDO, !first);
+          // dP^T = V dO^T (its TMEM region held dQ of the previous iteration)
+          if (!first) {
+            mbar_wait(dq_drained, (it_n - 1) & 1);
+            tc_fence_after();
+          }
+          issue_kmajor<D>(tmem + 128, sV, sDO);
+          tc_commit(dp_full);
+          tc_commit(do_empty);
+          // S^T of the next iteration (P^T of this one has been consumed by dV, in issue order)
+          if (has_next) {
+            mbar_wait(&q_full[(it_n + 1) & 1], ((it_n + 1) >> 1) & 1);
+            tc_fence_after();
+            issue_kmajor<D>(tmem, sK, sQ + ((it_n + 1) & 1) * L::kTileBytes);
+            tc_commit(s_full);
+          }
+          // dK += dS^T Q ; dQ = dS K
+          mbar_wait(ds_full, it_n & 1);
+          tc_fence_after();
+          issue_dk<D>(tmem + 256, sDS, sQ + st * L::kTileBytes, !first);
+          issue_dq<D>(tmem + 128, sDS, sK);
+          tc_commit(dq_full);
+          tc_commit(&q_empty[st]);
+          first = false;
+          ++it_n;
+          if (!has_next) break;
+          wk = nxt;
+        }
+        tc_commit(acc_full);
+        tc_commit(kv_empty);
+        ++item_n;
+      }
+    }
+  } else if (warp < 8) {
+    // ==================================== compute warpgroups ====================================
+    const int wg = warp >> 2;
+    const int r = threadIdx.x & 127;  // key row of the tile
+    const uint32_t lane_addr = uint32_t((warp & 3) * 32) << 16;
+    const uint32_t tS = tmem + lane_addr + wg * 64;         // this half's S^T columns (fp32)
+    const uint32_t tP = tS;                                  // its P^T (packed bf16), 32 columns
+    const uint32_t tDP = tmem + lane_addr + 128 + wg * 64;  // this half's dP^T columns
+    const uint32_t tDQ = tmem + lane_addr + 128 + wg * (D / 2);  // dQ columns drained by this WG
+    uint8_t* ds_row = smem + L::kDSOff + wg * (kTile * 128) + r * 128;
+    uint8_t* dq_stage = smem + L::kDQOff + wg * (kTile * 128);
+    uint32_t item_n = 0, it_n = 0;
+    for (int w = blockIdx.x; w < total_work; w += gridDim.x) {
+      const Item it = p.items[w / p.n_kv_heads];
+      const int g = w % p.n_kv_heads;
+      const int b = it.local0 + r;  // key index inside its range
+      const bool key_ok = b < it.range_len;
+      BwdWalker wk;
+      wk.init(p.spans, it, p.group);
+      __nv_bfloat16* out = (wg == 0 ? p.dK : p.dV) + ((int64_t)it.row0 + r) * p.kv_row_stride +
+                           (int64_t)g * D;
+      if (wk.done()) {  // no query sees this key tile: its gradients are zero
+        if (key_ok)
+          for (int c = 0; c < D / 8; ++c) reinterpret_cast<uint4*>(out)[c] = make_uint4(0, 0, 0, 0);
+        continue;
+      }
+      float P[64];
+      int prev_h = 0, prev_qrow = 0;
+      bool first = true;
+
+      auto compute_p = [&](const BwdWalker& k, uint32_t n) {
+        mbar_wait(s_full, n & 1);
+        tc_fence_after();
+        uint32_t s[64];
+        tmem_ld32(tS, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
+        tmem_ld32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
+        tmem_wait_ld();
+        const float* lse = lse_s + (n & 1) * kTile + wg * 64;
+        const int a0 = k.qi * kTile + wg * 64;  // query index of this half's first column
+        // column cc visible iff b <= a0 + cc + off
+        const bool full = it.local0 + kTile - 1 <= a0 + k.sp.off && it.local0 + kTile <= it.range_len;
+        const int c_min = key_ok ? b - k.sp.off - a0 : (1 << 30);
+#pragma unroll
+        for (int c4 = 0; c4 < 16; ++c4) {
+          const float4 l4 = *reinterpret_cast<const float4*>(lse + 4 * c4);
+          const float lv[4] = {l4.x, l4.y, l4.z, l4.w};
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const int cc = 4 * c4 + j;
+            float pv = ex2(fmaf(__uint_as_float(s[cc]), p.scale_log2, -lv[j]));
+            if (!full && cc < c_min) pv = 0.f;
+            P[cc] = pv;
+          }
+        }
+        uint32_t pk[32];
+#pragma unroll
+        for (int i = 0; i < 32; ++i) pk[i] = pack_bf16(P[2 * i], P[2 * i + 1]);
+        tmem_st32(tP, pk);
+        tmem_wait_st();
+        tc_fence_before();
+        mbar_arrive(p_full);
+      };
+
+      auto drain_dq = [&](uint32_t n) {  // dQ of iteration n -> smem -> TMA reduce-add
+        mbar_wait(dq_full, n & 1);
+        tc_fence_after();
+#pragma unroll
+        for (int c = 0; c < D / 64; ++c) {
+          uint32_t v[32];
+          tmem_ld32(tDQ + c * 32, v);
+          tmem_wait_ld();
+          if (c == D / 64 - 1) {
+            tc_fence_before();
+            mbar_arrive(dq_drained);
+          }
+          if (r == 0) bulk_wait_group_read<0>();  // the previous reduce has read the staging tile
+          bar_sync(1 + wg, 128);
+#pragma unroll
+          for (int j = 0; j < 8; ++j)
+            *reinterpret_cast<uint4*>(dq_stage + r * 128 + ((j ^ (r & 7)) * 16)) =
+                make_uint4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+          fence_proxy_async_smem();
+          bar_sync(1 + wg, 128);
+          if (r == 0) {
+            tma_reduce_add_3d(&tmDQ, dq_stage, wg * (D / 2) + c * 32, prev_h, prev_qrow);
+            bulk_commit_group();
+          }
+        }
+      };
+
+      compute_p(wk, it_n);
+      while (true) {
+        BwdWalker nxt = wk;
+        nxt.next();
+        const bool has_next = !nxt.done();
+        if (!first) drain_dq(it_n - 1);
+        // dS^T = P^T * (dP^T * scale - delta * scale)
+        mbar_wait(dp_full, it_n & 1);
+        tc_fence_after();
+        {
+          uint32_t dp[64];
+          tmem_ld32(tDP, *reinterpret_cast<uint32_t(*)[32]>(&dp[0]));
+          tmem_ld32(tDP + 32, *reinterpret_cast<uint32_t(*)[32]>(&dp[32]));
+          tmem_wait_ld();
+          const float* dl = delta_s + (it_n & 1) * kTile + wg * 64;
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {  // 8 queries = one 16-byte chunk of the dS^T row
+            const float4 d0 = *reinterpret_cast<const float4*>(dl + 8 * j);
+            const float4 d1 = *reinterpret_cast<const float4*>(dl + 8 * j + 4);
+            const float dv[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+            float ds[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e)
+              ds[e] = P[8 * j + e] * fmaf(__uint_as_float(dp[8 * j + e]), p.scale, -dv[e]);
+            uint4 pk;
+            pk.x = pack_bf16(ds[0], ds[1]);
+            pk.y = pack_bf16(ds[2], ds[3]);
+            pk.z = pack_bf16(ds[4], ds[5]);
+            pk.w = pack_bf16(ds[6], ds[7]);
+            *reinterpret_cast<uint4*>(ds_row + ((j ^ (r & 7)) * 16)) = pk;
+          }
+        }
+        fence_proxy_async_smem();
+        tc_fence_before();
+        mbar_arrive(ds_full);
+        prev_h = g * p.group + wk.hi;
+        prev_qrow = wk.q_row();
+        first = false;
+        ++it_n;
+        if (!has_next) break;
+        compute_p(nxt, it_n);
+        wk = nxt;
+      }
+      drain_dq(it_n - 1);
+      // ------------------------------ epilogue: dK (WG A), dV (WG B) ------------------------------
+      mbar_wait(acc_full, item_n & 1);
+      tc_fence_after();
+      const uint32_t tAcc = tmem + lane_addr + 256 + wg * 128;
+#pragma unroll
+      for (int c = 0; c < D / 32; ++c) {
+        uint32_t v[32];
+        tmem_ld32(tAcc + c * 32, v);
+        tmem_wait_ld();
+        if (key_ok) {
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            uint4 pk;
+            pk.x = pack_bf16(__uint_as_float(v[8 * q + 0]), __uint_as_float(v[8 * q + 1]));
+            pk.y = pack_bf16(__uint_as_float(v[8 * q + 2]), __uint_as_float(v[8 * q + 3]));
+            pk.z = pack_bf16(__uint_as_float(v[8 * q + 4]), __uint_as_float(v[8 * q + 5]));
+            pk.w = pack_bf16(__uint_as_float(v[8 * q + 6]), __uint_as_float(v[8 * q + 7]));
+            reinterpret_cast<uint4*>(out)[c * 4 + q] = pk;
+          }
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(acc_empty);
+      ++item_n;
+    }
+    if (r == 0) bulk_wait_group<0>();  // all dQ reductions have landed before the CTA exits
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 8) tmem_dealloc<512>(tmem);
+}
+
+}  // namespace
+
+extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, const void* K,
+                                   const void* V, const void* dO, const float* LSE_final,
+                                   const float* delta, const bs_seg_t* segs, int32_t n_segs,
+                                   float* dQ_acc, void* dK, void* dV, void* ws, size_t ws_bytes,
+                                   void* stream) {
+  bs_status_t rc = bs::validate_shape(shape, "bs_attn_bwd");
+  if (rc != BS_OK) return rc;
+  BS_REQUIRE(Q && K && V && dO && LSE_final && delta && dQ_acc && dK && dV, BS_ERR_INVALID_ARG,
+             "bs_attn_bwd: null tensor pointer");
+  BS_REQUIRE(n_segs >= 0 && (segs || n_segs == 0), BS_ERR_INVALID_ARG, "bs_attn_bwd: bad segs");
+  BS_REQUIRE((((uintptr_t)dK | (uintptr_t)dV | (uintptr_t)dQ_acc) & 15) == 0, BS_ERR_INVALID_ARG,
+             "bs_attn_bwd: output pointers must be 16-byte aligned");
+  if (shape->kv_rows == 0) return BS_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  bs::SchedTables tb;
+  rc = bs::build_bwd_tables(segs, n_segs, shape->q_rows, shape->kv_rows, &tb);
+  if (rc != BS_OK) return rc;
+  bs::WsLayout L;
+  rc = bs::upload_tables(tb, ws, ws_bytes, st, &L);
+  if (rc != BS_OK) return rc;
+  uint8_t* wsb = (uint8_t*)ws;
+  rc = bs::launch_fill_rows((const int2*)(wsb + L.fill_off), (int)tb.fill.size(), tb.max_fill_rows,
+                            dK, dV, nullptr, shape->n_kv_heads, shape->head_dim,
+                            shape->kv_row_stride, 0, st);
+  if (rc != BS_OK) return rc;
+  if (tb.items.empty()) return BS_OK;
+
+  const int D = shape->head_dim;
+  CUtensorMap tmQ, tmK, tmV, tmDO, tmDQ;
+  rc = bs::make_tensor_map_3d(&tmQ, Q, 2, D, shape->n_q_heads, shape->q_rows, shape->q_row_stride,
+                              64, bs::kTile, true);
+  if (rc != BS_OK) return rc;
+  rc = bs::make_tensor_map_3d(&tmDO, dO, 2, D, shape->n_q_heads, shape->q_rows,
+                              shape->q_row_stride, 64, bs::kTile, true);
+  if (rc != BS_OK) return rc;
+  rc = bs::make_tensor_map_3d(&tmK, K, 2, D, shape->n_kv_heads, shape->kv_rows,
+                              shape->kv_row_stride, 64, bs::kTile, true);
+  if (rc != BS_OK) return rc;
+  rc = bs::make_tensor_map_3d(&tmV, V, 2, D, shape->n_kv_heads, shape->kv_rows,
+                              shape->kv_row_stride, 64, bs::kTile, true);
+  if (rc != BS_OK) return rc;
+  rc = bs::make_tensor_map_3d(&tmDQ, dQ_acc, 4, D, shape->n_q_heads, shape->q_rows,
+                              (int64_t)shape->n_q_heads * D, 32, bs::kTile, true);
+  if (rc != BS_OK) return rc;
+
+  BwdParams p;
+  p.items = (const bs::Item*)(wsb + L.items_off);
+  p.spans = (const bs::Span*)(wsb + L.spans_off);
+  p.n_items = (int32_t)tb.items.size();
+  p.n_kv_heads = shape->n_kv_heads;
+  p.group = shape->n_q_heads / shape->n_kv_heads;
+  p.q_rows = shape->q_rows;
+  p.scale = shape->softmax_scale > 0.f ? shape->softmax_scale : 1.f / sqrtf((float)D);
+  p.scale_log2 = p.scale * 1.4426950408889634f;
+  p.LSE = LSE_final;
+  p.delta = delta;
+  p.lse_head_stride = shape->lse_head_stride;
+  p.dK = (__nv_bfloat16*)dK;
+  p.dV = (__nv_bfloat16*)dV;
+  p.kv_row_stride = shape->kv_row_stride;
+  const int64_t work = (int64_t)p.n_items * p.n_kv_heads;
+  const int grid = (int)(work < bs::sm_count() ? work : bs::sm_count());
+  if (D == 128) {
+    BS_CUDA(cudaFuncSetAttribute(attn_bwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 BwdSmem<128>::kBytes));
+    attn_bwd_kernel<128><<<grid, kBwdThreads, BwdSmem<128>::kBytes, st>>>(tmQ, tmK, tmV, tmDO, tmDQ, p);
+  } else {
+    BS_CUDA(cudaFuncSetAttribute(attn_bwd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 BwdSmem<64>::kBytes));
+    attn_bwd_kernel<64><<<grid, kBwdThreads, BwdSmem<64>::kBytes, st>>>(tmQ, tmK, tmV, tmDO, tmDQ, p);
+  }
+  BS_CUDA(cudaGetLastError());
+  bs::count_launch();
+  return BS_OK;
 }
