@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the driver.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Workload: BASELINE.json configs[1] (the 7B-shaped packed batch the metric is quoted on):
+32768-token buffer, log-normal document lengths, 32/32 heads, head_dim 128, bf16, fwd + bwd.
+A "step" is one pass of the whole hot path: bs_plan (host) -> bs_attn_fwd -> bs_attn_bwd_prep ->
+bs_attn_bwd -> bs_attn_bwd_finish (cfg2 has one ring step, so the LSE merge is not on its path;
+the merge is timed separately on the cfg3-shaped partials and reported under "merge").
+value = unmasked FLOPs (14 * D * Hq * visible pairs) of all ranks / max-over-ranks device time.
+N > 1: every rank runs its own cfg2-shaped batch (weak scaling, no data-path collective —
+HDP ranks are independent per micro-batch); torch.distributed is used only for
+the barrier and the max-over-ranks of the device time.
+--impl reference: times the fp64 oracle (the reference arm of this tier) on the host cores.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "varlen causal attn fwd+bwd TFLOP/s (unmasked)"
+WORKLOAD = "cfg2_7B_packed_32k"
+ORACLE_SAMPLE_HEADS = 1  # heads of cfg2 the oracle is timed on (MHA heads are independent)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return dict(tflops=d["bf16_tflops"], tflops_sustained=d.get("bf16_tflops_sustained"),
+                    hbm=d["hbm_gbs"], source="measured (MEASURED_PEAKS.json)")
+    return dict(tflops=1590.0, tflops_sustained=1400.0, hbm=6650.0,
+                source="fallback (B200_PROFILING.md)")
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag = index, [], set(), False
+        self.max_mhz = None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                     nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                     nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                     nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+            while not self.stop_flag:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                time.sleep(0.02)
+        except Exception as e:  # NVML missing: report nothing rather than fail the bench
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def result(self):
+        s = sorted(self.samples)
+        return dict(sm_mhz=s[len(s) // 2] if s else None, sm_max_mhz=self.max_mhz,
+                    reasons=sorted(self.reasons))
+
+
+def cfg2():
+    from paper_2502_21231_b200.synth import make_workload
+    return make_workload(2)
+
+
+def oracle_sample_run(w, heads, want_time=True):
+    """Oracle fwd + bwd on the first `heads` heads of cfg2 (all 32768 tokens).  Returns
+    (seconds, flops, threads)."""
+    import numpy as np
+    import oracle
+    from paper_2502_21231_b200.synth import rng, workloads
+    pl = oracle.oracle_plan(w.seqs)
+    D = w.head_dim
+    runs = workloads.runs_from(pl["q_seq"], pl["q_pos"])
+    full = w.n_q_heads * D
+
+    def gen(stream):
+        return workloads.gen_rows(w.seed, stream, runs, full).reshape(-1, w.n_q_heads, D)[:, :heads].copy()
+    Q, K, V, dO = gen(rng.STREAM_Q), gen(rng.STREAM_K), gen(rng.STREAM_V), gen(rng.STREAM_DO)
+    t0 = time.perf_counter()
+    oracle.attn_fwd(Q, K, V, pl["q_seq"], pl["q_pos"], pl["q_seq"], pl["q_pos"])
+    oracle.attn_bwd(Q, K, V, dO, pl["q_seq"], pl["q_pos"], pl["q_seq"], pl["q_pos"])
+    dt = time.perf_counter() - t0
+    pairs = pl["steps"][0]["visible_pairs"]
+    return dt, 14.0 * D * heads * pairs, oracle.threads()
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    w = cfg2()
+    times = []
+    for i in range(args.warmup + args.steps):
+        dt, flops, thr = oracle_sample_run(w, ORACLE_SAMPLE_HEADS)
+        if i >= args.warmup:
+            times.append(dt)
+    t = sum(times) / len(times)
+    val = flops / t / 1e12
+    sample = (f"{ORACLE_SAMPLE_HEADS} of {w.n_q_heads} heads of {WORKLOAD}, all 32768 tokens, "
+              "fwd+bwd, fp64")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "TFLOP/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "TFLOP/s", "cores": thr, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": val, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args, rank, world, local_rank):
+    import numpy as np
+    import torch
+    from paper_2502_21231_b200 import binding as B
+    from paper_2502_21231_b200.synth import rng, workloads
+
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    w = cfg2()
+    Hq, Hkv, D = w.n_q_heads, w.n_kv_heads, w.head_dim
+    seed = w.seed + 100 * rank  # same document lengths on every rank, different tensors
+    pl = B.plan(w.seqs)
+    st = pl["steps"][0]
+    rows, pairs = pl["q_rows"], st["visible_pairs"]
+    qruns = workloads.runs_from(pl["q_seq"], pl["q_pos"])
+
+    def host(stream, heads):
+        bits = workloads.gen_rows(seed, stream, qruns, heads * D)
+        return torch.from_numpy(bits.view(np.int16)).view(torch.bfloat16).view(rows, heads, D).pin_memory()
+    hQ, hK, hV, hdO = host(rng.STREAM_Q, Hq), host(rng.STREAM_K, Hkv), host(rng.STREAM_V, Hkv), host(rng.STREAM_DO, Hq)
+    Q, K, V, dO = (t.cuda() for t in (hQ, hK, hV, hdO))
+    O, dQ = torch.empty_like(Q), torch.empty_like(Q)
+    dK, dV = torch.empty_like(K), torch.empty_like(K)
+    LSE = torch.empty((Hq, rows), dtype=torch.float32, device="cuda")
+    delta = torch.empty_like(LSE)
+    acc = torch.empty((rows, Hq, D), dtype=torch.float32, device="cuda")
+    sh = B.make_shape(Hq, Hkv, D, rows, rows)
+    ws_f = torch.empty(B.attn_workspace_bytes(sh, len(st["segs"]), False), dtype=torch.uint8, device="cuda")
+    ws_b = torch.empty(B.attn_workspace_bytes(sh, len(st["segs"]), True), dtype=torch.uint8, device="cuda")
+    hO, hdQ, hdK, hdV = (torch.empty_like(t, device="cpu").pin_memory() for t in (O, dQ, dK, dV))
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+
+    def step(marks=None):
+        p = B.plan(w.seqs)["steps"][0]["segs"]  # a1: host planning is part of the step
+        if marks:
+            marks[0].record()
+        B.attn_fwd(sh, Q, K, V, p, (0, rows), O, LSE, ws_f)
+        if marks:
+            marks[1].record()
+        B.attn_bwd_prep(sh, O, dO, delta, acc)
+        if marks:
+            marks[2].record()
+        B.attn_bwd(sh, Q, K, V, dO, LSE, delta, p, acc, dK, dV, ws_b)
+        if marks:
+            marks[3].record()
+        B.attn_bwd_finish(sh, acc, dQ)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    marks = [[ev() for _ in range(4)] for _ in range(args.steps)]
+    B.launch_count_reset()
+    e0, e1 = ev(), ev()
+    e0.record()
+    for i in range(args.steps):
+        step(marks[i])
+    e1.record()
+    barrier()
+    launches = B.launch_count()
+    ms = e0.elapsed_time(e1)
+    t_fwd = sum(m[0].elapsed_time(m[1]) for m in marks) / args.steps
+    t_bwd = sum(m[2].elapsed_time(m[3]) for m in marks) / args.steps
+    # end to end: pinned host inputs -> device, the step, results -> host, all inside the region
+    for _ in range(2):
+        for d, h in ((Q, hQ), (K, hK), (V, hV), (dO, hdO)):
+            d.copy_(h, non_blocking=True)
+        step()
+    barrier()
+    f0, f1 = ev(), ev()
+    f0.record()
+    for _ in range(args.steps):
+        for d, h in ((Q, hQ), (K, hK), (V, hV), (dO, hdO)):
+            d.copy_(h, non_blocking=True)
+        step()
+        for h, d in ((hO, O), (hdQ, dQ), (hdK, dK), (hdV, dV)):
+            h.copy_(d, non_blocking=True)
+    f1.record()
+    barrier()
+    ms_e2e = f0.elapsed_time(f1)
+    sampler.stop_flag = True
+    sampler.join()
+    if dist:
+        t = torch.tensor([ms, ms_e2e], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, ms_e2e = t.tolist()
+    flops_step = 14.0 * D * Hq * pairs
+    out = None
+    if rank == 0:
+        pk = peaks()
+        nb = lambda t: t.numel() * t.element_size()  # noqa: E731
+        merge = bench_merge(B, torch, pk)
+        dt, fl, thr = oracle_sample_run(w, ORACLE_SAMPLE_HEADS)
+        bwd_tflops = 10.0 * D * Hq * pairs / (t_bwd * 1e-3) / 1e12
+        out = {
+            "metric": METRIC, "value": world * flops_step * args.steps / (ms * 1e-3) / 1e12,
+            "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "tokens": rows, "documents": len(w.seqs),
+                       "n_q_heads": Hq, "n_kv_heads": Hkv, "head_dim": D,
+                       "visible_pairs_per_head": pairs, "flops_per_step": flops_step,
+                       "l2": "inputs+outputs 2.4 GB per step exceed the 126 MB L2; no flush",
+                       "peaks": pk["source"]},
+            "pct_of_bf16_peak": {"measured_burst": 100 * flops_step * args.steps / (ms * 1e-3) / 1e12 / pk["tflops"],
+                                 "nominal_2250": 100 * flops_step * args.steps / (ms * 1e-3) / 1e12 / 2250.0},
+            "kernels_ms": {"bs_attn_fwd": t_fwd, "bs_attn_bwd": t_bwd,
+                           "fwd_tflops": 4.0 * D * Hq * pairs / (t_fwd * 1e-3) / 1e12,
+                           "bwd_tflops": bwd_tflops},
+            "roofline": {"kernel": "attn_bwd_kernel<128>", "bound": "tensor", "achieved": bwd_tflops,
+                         "peak": pk["tflops"], "unit": "TFLOP/s", "frac": bwd_tflops / pk["tflops"],
+                         "traffic": None},
+            "merge": merge,
+            "cpu_baseline": {"value": fl / dt / 1e12, "unit": "TFLOP/s", "cores": thr, "kind": "oracle",
+                             "sample": f"{ORACLE_SAMPLE_HEADS} of {Hq} heads of {WORKLOAD}, all "
+                                       f"{rows} tokens, fwd+bwd, fp64, {dt:.1f} s"},
+            "e2e": {"value": world * flops_step * args.steps / (ms_e2e * 1e-3) / 1e12, "unit": "TFLOP/s",
+                    "h2d_bytes_per_step": sum(nb(t) for t in (Q, K, V, dO)),
+                    "d2h_bytes_per_step": sum(nb(t) for t in (O, dQ, dK, dV))},
+            "gpu_launches": launches, "clocks": sampler.result()}
+    if dist:
+        dist.barrier()
+        dist.destroy_process_group()
+    if out:
+        print(json.dumps(out))
+
+
+def bench_merge(B, torch, pk):
+    """bs_lse_merge on the cfg3-shaped partials: n = 8, 32768 rows x 64 heads x 128 (4.6 GB)."""
+    n, rows, Hq, D = 8, 32768, 64, 128
+    Os = [torch.randn((rows, Hq, D), device="cuda").to(torch.bfloat16) for _ in range(n)]
+    Ls = [torch.randn((Hq, rows), device="cuda") for _ in range(n)]
+    O, L = torch.empty_like(Os[0]), torch.empty_like(Ls[0])
+    sh = B.make_shape(Hq, 8, D, rows, rows)
+    for _ in range(3):
+        B.lse_merge(Os, Ls, sh, (0, rows), O, L)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    it = 10
+    e0.record()
+    for _ in range(it):
+        B.lse_merge(Os, Ls, sh, (0, rows), O, L)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / it
+    nbytes = (n + 1) * rows * Hq * (2 * D + 4)
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    return {"workload": "cfg3 partials: n=8, 32768 rows, 64 heads, D=128", "ms": ms, "bytes": nbytes,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s",
+                         "frac": gbs / pk["hbm"], "frac_of_nominal_8000": gbs / 8000.0, "traffic": None}}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    local_rank = int(os.environ.get("LOCAL_RANK", 0))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -133,7 +133,11 @@ int oracle_attn_fwd(int64_t nq, int64_t nk, int Hq, int Hkv, int D, const uint16
  * (the plain definition).  When given (the merged LSE and delta of a larger key set), the
  * result is this key set's exact share of the gradients of attention over the larger set
  * (reading 13; the sum over a partition of the keys equals the full backward, which
- * tests/test_oracle_attn.py checks). */
+ * tests/test_oracle_attn.py checks).
+ * Written as the formulas read: pass A, one query row (h,i) at a time: LSE_i, delta_i and
+ * dQ[i,h,:] = scale sum_j dS_ij K[j,g,:];  pass B, one key row (g,j) at a time:
+ * dV[j,g,:] = sum_{h in g} sum_i P_ij dO[i,h,:] and dK[j,g,:] = scale sum_{h in g} sum_i dS_ij
+ * Q[i,h,:].  Each output row is owned by one loop iteration, so the loops parallelise as is. */
 int oracle_attn_bwd(int64_t nq, int64_t nk, int Hq, int Hkv, int D, const uint16_t* Q,
                     const uint16_t* K, const uint16_t* V, const uint16_t* dO, const int32_t* q_seq,
                     const int32_t* q_pos, const int32_t* k_seq, const int32_t* k_pos, double scale,
@@ -141,6 +145,13 @@ int oracle_attn_bwd(int64_t nq, int64_t nk, int Hq, int Hkv, int D, const uint16
                     double* dV) {
   int fail = 0;
   const int G = Hq / Hkv;
+  double* LSE = (double*)malloc(sizeof(double) * (size_t)(nq * Hq > 0 ? nq * Hq : 1));
+  double* delta = (double*)malloc(sizeof(double) * (size_t)(nq * Hq > 0 ? nq * Hq : 1));
+  if (!LSE || !delta) {
+    free(LSE);
+    free(delta);
+    return -1;
+  }
   memset(dQ, 0, sizeof(double) * (size_t)nq * Hq * D);
   memset(dK, 0, sizeof(double) * (size_t)nk * Hkv * D);
   memset(dV, 0, sizeof(double) * (size_t)nk * Hkv * D);
@@ -154,21 +165,20 @@ int oracle_attn_bwd(int64_t nq, int64_t nk, int Hq, int Hkv, int D, const uint16
     }
 #pragma omp barrier
     if (!fail) {
-      /* one kv head per thread at a time: dK/dV rows of head g are touched by one thread only */
-#pragma omp for schedule(dynamic, 1)
-      for (int g = 0; g < Hkv; ++g) {
-        for (int h = g * G; h < (g + 1) * G; ++h) {
-          for (int64_t i = 0; i < nq; ++i) {
-            double m;
-            int64_t cnt = scores_row(nk, Hq, Hkv, D, Q, K, q_seq, q_pos, k_seq, k_pos, scale, h,
-                                     i, s, &m);
-            if (cnt == 0) continue;
-            const uint16_t* q = Q + ((size_t)i * Hq + h) * D;
-            const uint16_t* go = dO + ((size_t)i * Hq + h) * D;
-            double lse, delta;
+      /* pass A: per query row */
+#pragma omp for collapse(2) schedule(dynamic, 16)
+      for (int h = 0; h < Hq; ++h) {
+        for (int64_t i = 0; i < nq; ++i) {
+          const int g = h / G;
+          double m;
+          int64_t cnt =
+              scores_row(nk, Hq, Hkv, D, Q, K, q_seq, q_pos, k_seq, k_pos, scale, h, i, s, &m);
+          double lse = -INFINITY, dl = 0.0;
+          const uint16_t* go = dO + ((size_t)i * Hq + h) * D;
+          if (cnt > 0) {
             if (LSE_in) {
               lse = LSE_in[(size_t)h * nq + i];
-              delta = delta_in[(size_t)h * nq + i];
+              dl = delta_in[(size_t)h * nq + i];
             } else {
               double l = 0.0;
               for (int64_t j = 0; j < nk; ++j)
@@ -181,8 +191,7 @@ int oracle_attn_bwd(int64_t nq, int64_t nk, int Hq, int Hkv, int D, const uint16
                 const uint16_t* v = V + ((size_t)j * Hkv + g) * D;
                 for (int d = 0; d < D; ++d) o[d] += p * bf16_to_f64(v[d]);
               }
-              delta = 0.0;
-              for (int d = 0; d < D; ++d) delta += bf16_to_f64(go[d]) * o[d];
+              for (int d = 0; d < D; ++d) dl += bf16_to_f64(go[d]) * o[d];
             }
             double* dq = dQ + ((size_t)i * Hq + h) * D;
             for (int64_t j = 0; j < nk; ++j) {
@@ -190,14 +199,38 @@ int oracle_attn_bwd(int64_t nq, int64_t nk, int Hq, int Hkv, int D, const uint16
               const double p = exp(s[j] - lse);
               const uint16_t* k = K + ((size_t)j * Hkv + g) * D;
               const uint16_t* v = V + ((size_t)j * Hkv + g) * D;
-              double* dk = dK + ((size_t)j * Hkv + g) * D;
-              double* dv = dV + ((size_t)j * Hkv + g) * D;
               double dp = 0.0;
               for (int d = 0; d < D; ++d) dp += bf16_to_f64(go[d]) * bf16_to_f64(v[d]);
-              const double ds = p * (dp - delta);
+              const double ds = p * (dp - dl);
+              for (int d = 0; d < D; ++d) dq[d] += scale * ds * bf16_to_f64(k[d]);
+            }
+          }
+          LSE[(size_t)h * nq + i] = lse;
+          delta[(size_t)h * nq + i] = dl;
+        }
+      }
+      /* pass B: per key row (implicit barrier of the omp-for above orders the two passes) */
+#pragma omp for collapse(2) schedule(dynamic, 16)
+      for (int g = 0; g < Hkv; ++g) {
+        for (int64_t j = 0; j < nk; ++j) {
+          const uint16_t* k = K + ((size_t)j * Hkv + g) * D;
+          const uint16_t* v = V + ((size_t)j * Hkv + g) * D;
+          double* dk = dK + ((size_t)j * Hkv + g) * D;
+          double* dv = dV + ((size_t)j * Hkv + g) * D;
+          for (int h = g * G; h < (g + 1) * G; ++h) {
+            for (int64_t i = 0; i < nq; ++i) {
+              if (!visible(q_seq, q_pos, k_seq, k_pos, i, j)) continue;
+              const uint16_t* q = Q + ((size_t)i * Hq + h) * D;
+              const uint16_t* go = dO + ((size_t)i * Hq + h) * D;
+              double acc = 0.0, dp = 0.0;
+              for (int d = 0; d < D; ++d) {
+                acc += bf16_to_f64(q[d]) * bf16_to_f64(k[d]);
+                dp += bf16_to_f64(go[d]) * bf16_to_f64(v[d]);
+              }
+              const double p = exp(scale * acc - LSE[(size_t)h * nq + i]);
+              const double ds = p * (dp - delta[(size_t)h * nq + i]);
               for (int d = 0; d < D; ++d) {
                 dv[d] += p * bf16_to_f64(go[d]);
-                dq[d] += scale * ds * bf16_to_f64(k[d]);
                 dk[d] += scale * ds * bf16_to_f64(q[d]);
               }
             }
@@ -208,6 +241,8 @@ int oracle_attn_bwd(int64_t nq, int64_t nk, int Hq, int Hkv, int D, const uint16
     free(s);
     free(o);
   }
+  free(LSE);
+  free(delta);
   return fail ? -1 : 0;
 }
 
