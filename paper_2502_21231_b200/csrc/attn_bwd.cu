@@ -25,6 +25,7 @@
 #include "common.h"
 #include "launch_utils.h"
 #include "ptx.cuh"
+#include "sched.cuh"
 #include "worklist.h"
 
 namespace {
@@ -36,9 +37,7 @@ constexpr int kBwdThreads = 384;
 constexpr int kComputeThreads = 256;
 
 struct BwdParams {
-  const Item* items;
-  const Span* spans;
-  int32_t n_items;  // key-tile items (x n_kv_heads work items)
+  SchedView sv;     // units = key-tile items x n_kv_heads
   int32_t n_kv_heads, group;
   int32_t q_rows;
   float scale, scale_log2;
@@ -66,7 +65,8 @@ struct BwdSmem {
   // dq_drained acc_full acc_empty
   static constexpr int kNumBars = 16;
   static constexpr int kTmemSlotOff = kBarOff + kNumBars * 8;
-  static constexpr int kBytes = kTmemSlotOff + 16;
+  static constexpr int kSchedOff = kTmemSlotOff + 16;
+  static constexpr int kBytes = kSchedOff + 64;
 };
 
 // Iterations of one item: for each query head of the group, for each span (query range), the
@@ -182,6 +182,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kTmemSlotOff);
   float* lse_s = reinterpret_cast<float*>(smem + L::kLseOff);
   float* delta_s = reinterpret_cast<float*>(smem + L::kDeltaOff);
+  SchedRing* sched = reinterpret_cast<SchedRing*>(smem + L::kSchedOff);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0 && (smem_u32(smem) & 1023u) != 0) {
@@ -189,6 +190,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     __trap();
   }
   if (warp == 9 && lane == 0) {
+    sched_ring_init(sched, kComputeThreads + 1);  // consumers: compute threads + the MMA lane
     mbar_init(kv_full, 1);
     mbar_init(kv_empty, 1);
     for (int i = 0; i < 2; ++i) {
@@ -220,16 +222,21 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   const uint32_t sK = smem_u32(smem + L::kKOff), sV = smem_u32(smem + L::kVOff);
   const uint32_t sQ = smem_u32(smem + L::kQOff), sDO = smem_u32(smem + L::kDOOff);
   const uint32_t sDS = smem_u32(smem + L::kDSOff);
-  const int total_work = p.n_items * p.n_kv_heads;
 
   if (warp == 9) {
     // ============================ TMA producer + LSE/delta staging ============================
     uint32_t item_n = 0, it_n = 0;  // items / iterations issued so far (ring phases)
-    for (int w = blockIdx.x; w < total_work; w += gridDim.x) {
-      const Item it = p.items[w / p.n_kv_heads];
-      const int g = w % p.n_kv_heads;
+    UnitProducer prod{sched};
+    while (true) {
+      int32_t w = 0;
+      if (lane == 0) w = prod.next(p.sv);
+      w = __shfl_sync(0xffffffffu, w, 0);
+      if (w < 0) break;
+      const Unit u = decode_unit(p.sv, w);
+      const Item& it = u.item;
+      const int g = u.head;
       BwdWalker wk;
-      wk.init(p.spans, it, p.group);
+      wk.init(p.sv.spans, it, p.group);
       if (wk.done()) continue;
       if (lane == 0) {
         mbar_wait(kv_empty, (item_n & 1) ^ 1);
@@ -271,10 +278,13 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     // ======================================= MMA issuer =======================================
     if (lane == 0) {
       uint32_t item_n = 0, it_n = 0;
-      for (int w = blockIdx.x; w < total_work; w += gridDim.x) {
-        const Item it = p.items[w / p.n_kv_heads];
+      UnitConsumer cons{sched};
+      int32_t w;
+      while ((w = cons.next()) >= 0) {
+        const Unit u = decode_unit(p.sv, w);
+        const Item& it = u.item;
         BwdWalker wk;
-        wk.init(p.spans, it, p.group);
+        wk.init(p.sv.spans, it, p.group);
         if (wk.done()) continue;
         mbar_wait(kv_full, item_n & 1);
         mbar_wait(acc_empty, (item_n & 1) ^ 1);  // previous item's dK/dV have left TMEM
@@ -339,13 +349,16 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint8_t* ds_row = smem + L::kDSOff + wg * (kTile * 128) + r * 128;
     uint8_t* dq_stage = smem + L::kDQOff + wg * (kTile * 128);
     uint32_t item_n = 0, it_n = 0;
-    for (int w = blockIdx.x; w < total_work; w += gridDim.x) {
-      const Item it = p.items[w / p.n_kv_heads];
-      const int g = w % p.n_kv_heads;
+    UnitConsumer cons{sched};
+    int32_t w;
+    while ((w = cons.next()) >= 0) {
+      const Unit u = decode_unit(p.sv, w);
+      const Item& it = u.item;
+      const int g = u.head;
       const int b = it.local0 + r;  // key index inside its range
       const bool key_ok = b < it.range_len;
       BwdWalker wk;
-      wk.init(p.spans, it, p.group);
+      wk.init(p.sv.spans, it, p.group);
       __nv_bfloat16* out = (wg == 0 ? p.dK : p.dV) + ((int64_t)it.row0 + r) * p.kv_row_stride +
                            (int64_t)g * D;
       if (wk.done()) {  // no query sees this key tile: its gradients are zero
@@ -361,8 +374,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_wait(s_full, n & 1);
         tc_fence_after();
         uint32_t s[64];
-        tmem_ld32(tS, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
-        tmem_ld32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
+        tmem_ld32(tS, &s[0]);
+        tmem_ld32(tS + 32, &s[32]);
         tmem_wait_ld();
         const float* lse = lse_s + (n & 1) * kTile + wg * 64;
         const int a0 = k.qi * kTile + wg * 64;  // query index of this half's first column
@@ -428,8 +441,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tc_fence_after();
         {
           uint32_t dp[64];
-          tmem_ld32(tDP, *reinterpret_cast<uint32_t(*)[32]>(&dp[0]));
-          tmem_ld32(tDP + 32, *reinterpret_cast<uint32_t(*)[32]>(&dp[32]));
+          tmem_ld32(tDP, &dp[0]);
+          tmem_ld32(tDP + 32, &dp[32]);
           tmem_wait_ld();
           const float* dl = delta_s + (it_n & 1) * kTile + wg * 64;
 #pragma unroll
@@ -510,7 +523,7 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   if (shape->kv_rows == 0) return BS_OK;
   cudaStream_t st = (cudaStream_t)stream;
   bs::SchedTables tb;
-  rc = bs::build_bwd_tables(segs, n_segs, shape->q_rows, shape->kv_rows, &tb);
+  rc = bs::build_bwd_tables(segs, n_segs, shape->q_rows, shape->kv_rows, shape->n_kv_heads, &tb);
   if (rc != BS_OK) return rc;
   bs::WsLayout L;
   rc = bs::upload_tables(tb, ws, ws_bytes, st, &L);
@@ -541,9 +554,7 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   if (rc != BS_OK) return rc;
 
   BwdParams p;
-  p.items = (const bs::Item*)(wsb + L.items_off);
-  p.spans = (const bs::Span*)(wsb + L.spans_off);
-  p.n_items = (int32_t)tb.items.size();
+  p.sv = bs::make_sched_view(wsb, L, tb, shape->n_kv_heads);
   p.n_kv_heads = shape->n_kv_heads;
   p.group = shape->n_q_heads / shape->n_kv_heads;
   p.q_rows = shape->q_rows;
@@ -555,8 +566,7 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   p.dK = (__nv_bfloat16*)dK;
   p.dV = (__nv_bfloat16*)dV;
   p.kv_row_stride = shape->kv_row_stride;
-  const int64_t work = (int64_t)p.n_items * p.n_kv_heads;
-  const int grid = (int)(work < bs::sm_count() ? work : bs::sm_count());
+  const int grid = tb.n_units < bs::sm_count() ? tb.n_units : bs::sm_count();
   if (D == 128) {
     BS_CUDA(cudaFuncSetAttribute(attn_bwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  BwdSmem<128>::kBytes));

@@ -1,11 +1,11 @@
 // attn_fwd.cu — bs_attn_fwd: one Q-chunk x KV-chunk step of packed varlen / zigzag-CP causal
 // attention on sm_100a (SURVEY.md 8(a) a2+a3; flash attention = exact attention).
 //
-// Kernel shape (one persistent CTA per SM, 320 threads):
+// Kernel shape (one persistent CTA per SM, 384 threads, registers re-split by setmaxnreg):
 //   warps 0-3  softmax warpgroup of Q tile 0   (thread r <-> row r of the 128-row tile)
 //   warps 4-7  softmax warpgroup of Q tile 1
 //   warp  8    MMA issuer (one elected lane): tcgen05.mma, accumulators in TMEM
-//   warp  9    TMA producer: Q once per item, K/V blocks through a 4-stage smem ring
+//   warp  9    TMA producer: Q per item and tile, K/V blocks through a 4-stage smem ring
 // A work item is (up to 256 query rows = two 128-row tiles of one query range, one query head).
 // TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,256+D) O1 [384,384+D); P (bf16) overwrites
 // the first 64 columns of its S.  Per KV block the tensor pipe runs, in issue order,
@@ -20,6 +20,7 @@
 #include "common.h"
 #include "launch_utils.h"
 #include "ptx.cuh"
+#include "sched.cuh"
 #include "worklist.h"
 
 namespace {
@@ -27,15 +28,14 @@ namespace {
 using namespace bs;
 using namespace bs::ptx;
 
-constexpr int kFwdThreads = 320;
+constexpr int kFwdThreads = 384;      // 2 softmax warpgroups + 1 auxiliary warpgroup (MMA, TMA)
+constexpr int kRegsSoftmax = 208;     // setmaxnreg budgets: 256 * 208 + 128 * 88 = 384 * 168
+constexpr int kRegsAux = 88;
 constexpr int kStages = 4;              // K/V ring depth (K and V blocks alternate in the ring)
 constexpr float kRescaleThreshold = 8.f;  // log2 units
 
 struct FwdParams {
-  const Item* items;
-  const Span* spans;
-  int32_t* counter;
-  int32_t n_items;  // query items (x n_q_heads work items)
+  SchedView sv;     // units = query items x n_q_heads
   int32_t n_q_heads, group;  // group = Hq / Hkv
   int32_t q_rows;
   float scale_log2;  // softmax_scale * log2(e)
@@ -50,11 +50,11 @@ struct FwdSmem {
   static constexpr int kQOff = 0;                   // 2 Q tiles
   static constexpr int kKVOff = 2 * kTileBytes;     // kStages K/V tiles
   static constexpr int kBarOff = kKVOff + kStages * kTileBytes;
-  // barriers: q_full, q_empty, kv_full[S], kv_empty[S], s_full[2], p_full[2], o_full[2]
-  static constexpr int kNumBars = 2 + 2 * kStages + 6;
+  // barriers: q_full[2], q_empty[2], kv_full[S], kv_empty[S], s_full[2], p_full[2], o_full[2]
+  static constexpr int kNumBars = 4 + 2 * kStages + 6;
   static constexpr int kTmemSlotOff = kBarOff + kNumBars * 8;
-  static constexpr int kItemOff = kTmemSlotOff + 8;  // broadcast slot for the dynamic scheduler
-  static constexpr int kBytes = kItemOff + 16;
+  static constexpr int kSchedOff = kTmemSlotOff + 8;  // SchedRing of the dynamic scheduler
+  static constexpr int kBytes = kSchedOff + 64;
   static constexpr int kAlloc = kBytes + 1024;  // slack to align the base to 1024 B
 };
 
@@ -154,27 +154,29 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
                                              ~uintptr_t(1023));
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::kBarOff);
-  uint64_t* q_full = bars;
-  uint64_t* q_empty = bars + 1;
-  uint64_t* kv_full = bars + 2;
-  uint64_t* kv_empty = bars + 2 + kStages;
-  uint64_t* s_full = bars + 2 + 2 * kStages;
+  uint64_t* q_full = bars;       // [2] per Q tile
+  uint64_t* q_empty = bars + 2;  // [2]
+  uint64_t* kv_full = bars + 4;
+  uint64_t* kv_empty = bars + 4 + kStages;
+  uint64_t* s_full = bars + 4 + 2 * kStages;
   uint64_t* p_full = s_full + 2;
   uint64_t* o_full = p_full + 2;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kTmemSlotOff);
+  SchedRing* sched = reinterpret_cast<SchedRing*>(smem + L::kSchedOff);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 9 && lane == 0) {
-    mbar_init(q_full, 1);
-    mbar_init(q_empty, 1);
-    for (int i = 0; i < kStages; ++i) {
-      mbar_init(&kv_full[i], 1);
-      mbar_init(&kv_empty[i], 1);
-    }
+    sched_ring_init(sched, 2 * kTile + 1);  // consumers: 256 softmax threads + the MMA lane
     for (int t = 0; t < 2; ++t) {
+      mbar_init(&q_full[t], 1);
+      mbar_init(&q_empty[t], 1);
       mbar_init(&s_full[t], 1);
       mbar_init(&p_full[t], kTile);
       mbar_init(&o_full[t], 1);
+    }
+    for (int i = 0; i < kStages; ++i) {
+      mbar_init(&kv_full[i], 1);
+      mbar_init(&kv_empty[i], 1);
     }
     fence_barrier_init();
     prefetch_tensormap(&tmQ);
@@ -187,27 +189,25 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
   const uint32_t smem_q = smem_u32(smem + L::kQOff), smem_kv = smem_u32(smem + L::kKVOff);
-  const int total_work = p.n_items * p.n_q_heads;
 
-  if (warp == 9) {
-    // ===================================== TMA producer =====================================
-    if (lane == 0) {
-      uint32_t q_ph = 0;
+  if (warp >= 8) {
+    setmaxnreg_dec<kRegsAux>();
+    if (warp == 9 && lane == 0) {
+      // ===================================== TMA producer =====================================
+      uint32_t q_ph[2] = {0, 0};
       Ring ring;
-      for (int w = blockIdx.x; w < total_work; w += gridDim.x) {
-        const Item it = p.items[w / p.n_q_heads];
-        const int h = w % p.n_q_heads, g = h / p.group;
+      UnitProducer prod{sched};
+      int32_t w;
+      while ((w = prod.next(p.sv)) >= 0) {
+        const Unit u = decode_unit(p.sv, w);
+        const Item& it = u.item;
+        const int h = u.head, g = h / p.group;
         Walker wk;
-        wk.init(p.spans, it);
+        wk.init(p.sv.spans, it);
         if (wk.done()) continue;
-        mbar_wait(q_empty, q_ph ^ 1);
-        q_ph ^= 1;
-        mbar_arrive_expect_tx(q_full, 2 * L::kTileBytes);
-        for (int t = 0; t < 2; ++t)
-          for (int half = 0; half < D / 64; ++half)
-            tma_load_3d(smem + L::kQOff + t * L::kTileBytes + half * (kTile * 128), &tmQ, q_full,
-                        half * 64, h, it.row0 + t * kTile);
-        for (; !wk.done(); wk.next()) {
+        // the first K/V block goes out before the Q tiles: the ring usually has room while the
+        // Q buffers are still held by the previous unit's last S MMAs
+        for (bool first = true; !wk.done(); wk.next(), first = false) {
           const int krow = wk.sp.begin + wk.j * kTile;
           for (int kv = 0; kv < 2; ++kv) {
             mbar_wait(&kv_empty[ring.stage], ring.phase ^ 1);
@@ -217,32 +217,51 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                           kv == 0 ? &tmK : &tmV, &kv_full[ring.stage], half * 64, g, krow);
             ring.advance();
           }
+          if (first) {
+            for (int t = 0; t < 2; ++t) {
+              if (wk.total(t) == 0) continue;
+              mbar_wait(&q_empty[t], q_ph[t] ^ 1);
+              q_ph[t] ^= 1;
+              mbar_arrive_expect_tx(&q_full[t], L::kTileBytes);
+              for (int half = 0; half < D / 64; ++half)
+                tma_load_3d(smem + L::kQOff + t * L::kTileBytes + half * (kTile * 128), &tmQ,
+                            &q_full[t], half * 64, h, it.row0 + t * kTile);
+            }
+          }
         }
       }
-    }
-  } else if (warp == 8) {
-    // ====================================== MMA issuer ======================================
-    if (lane == 0) {
-      uint32_t q_ph = 0, p_ph[2] = {0, 0};
+    } else if (warp == 8 && lane == 0) {
+      // ====================================== MMA issuer ======================================
+      uint32_t q_ph[2] = {0, 0}, p_ph[2] = {0, 0};
       Ring ring;
-      for (int w = blockIdx.x; w < total_work; w += gridDim.x) {
-        const Item it = p.items[w / p.n_q_heads];
+      UnitConsumer cons{sched};
+      int32_t w;
+      while ((w = cons.next()) >= 0) {
+        const Unit u = decode_unit(p.sv, w);
+        const Item& it = u.item;
         Walker cur;
-        cur.init(p.spans, it);
+        cur.init(p.sv.spans, it);
         if (cur.done()) continue;
         const int tot[2] = {cur.total(0), cur.total(1)};
-        int cnt[2] = {0, 0};
-        mbar_wait(q_full, q_ph);
-        q_ph ^= 1;
-        // prologue: S_t(0) = Q_t K_0^T
+        int n_s[2] = {0, 0}, n_pv[2] = {0, 0};
+        // S_t = Q_t K^T of one block; the first one of an item waits for the tile's Q, the last
+        // one releases the tile's Q buffer to the producer (next item's Q streams in early)
+        auto issue_s = [&](int t, uint32_t k_stage) {
+          if (n_s[t] == 0) {
+            mbar_wait(&q_full[t], q_ph[t]);
+            q_ph[t] ^= 1;
+            tc_fence_after();
+          }
+          issue_qk<D>(tmem + t * kTile, smem_q + t * L::kTileBytes,
+                      smem_kv + k_stage * L::kTileBytes);
+          tc_commit(&s_full[t]);
+          if (++n_s[t] == tot[t]) tc_commit(&q_empty[t]);
+        };
+        // prologue: S_t(0)
         mbar_wait(&kv_full[ring.stage], ring.phase);
         tc_fence_after();
         for (int t = 0; t < 2; ++t)
-          if (cur.active(t)) {
-            issue_qk<D>(tmem + t * kTile, smem_q + t * L::kTileBytes,
-                        smem_kv + ring.stage * L::kTileBytes);
-            tc_commit(&s_full[t]);
-          }
+          if (cur.active(t)) issue_s(t, ring.stage);
         tc_commit(&kv_empty[ring.stage]);
         ring.advance();
         while (true) {
@@ -264,36 +283,36 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
               p_ph[t] ^= 1;
               tc_fence_after();
               issue_pv<D>(tmem + 256 + t * kTile, tmem + t * kTile,
-                          smem_kv + v_stage * L::kTileBytes, cnt[t] > 0);
-              if (++cnt[t] == tot[t]) tc_commit(&o_full[t]);
+                          smem_kv + v_stage * L::kTileBytes, n_pv[t] > 0);
+              if (++n_pv[t] == tot[t]) tc_commit(&o_full[t]);
             }
-            if (has_next && nxt.active(t)) {
-              issue_qk<D>(tmem + t * kTile, smem_q + t * L::kTileBytes,
-                          smem_kv + k_stage * L::kTileBytes);
-              tc_commit(&s_full[t]);
-            }
+            if (has_next && nxt.active(t)) issue_s(t, k_stage);
           }
           tc_commit(&kv_empty[v_stage]);
           if (!has_next) break;
           tc_commit(&kv_empty[k_stage]);
           cur = nxt;
         }
-        tc_commit(q_empty);
       }
     }
   } else {
     // ================================== softmax warpgroups ==================================
+    setmaxnreg_inc<kRegsSoftmax>();
     const int t = warp >> 2;            // Q tile of this warpgroup
     const int r = threadIdx.x & 127;    // row of the tile owned by this thread
     const uint32_t lane_addr = uint32_t((warp & 3) * 32) << 16;
     const uint32_t tS = tmem + lane_addr + t * kTile;        // S_t, and P_t over its first 64 cols
     const uint32_t tO = tmem + lane_addr + 256 + t * kTile;  // O_t
+    const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
     uint32_t s_ph = 0, o_ph = 0;
-    for (int w = blockIdx.x; w < total_work; w += gridDim.x) {
-      const Item it = p.items[w / p.n_q_heads];
-      const int h = w % p.n_q_heads;
+    UnitConsumer cons{sched};
+    int32_t w;
+    while ((w = cons.next()) >= 0) {
+      const Unit u = decode_unit(p.sv, w);
+      const Item& it = u.item;
+      const int h = u.head;
       Walker wk;
-      wk.init(p.spans, it);
+      wk.init(p.sv.spans, it);
       const int at0 = wk.at0[t];
       const bool valid = r < wk.rows[t];
       const int64_t grow = (int64_t)it.row0 + t * kTile + r;
@@ -306,47 +325,46 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
         continue;
       }
-      float m_used = -CUDART_INF_F, l = 0.f;
+      float m_used = -CUDART_INF_F;
+      float2 l2 = make_float2(0.f, 0.f);
       int cnt = 0;
       for (; !wk.done(); wk.next()) {
         if (!wk.active(t)) continue;
         mbar_wait(&s_full[t], s_ph);
         s_ph ^= 1;
         tc_fence_after();
-        uint32_t s[kTile];
-        {
-          uint32_t(&s0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&s[0]);
-          uint32_t(&s1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&s[32]);
-          uint32_t(&s2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&s[64]);
-          uint32_t(&s3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&s[96]);
-          tmem_ld32(tS, s0);
-          tmem_ld32(tS + 32, s1);
-          tmem_ld32(tS + 64, s2);
-          tmem_ld32(tS + 96, s3);
-          tmem_wait_ld();
-        }
+        float s[kTile];
+        tmem_ld32(tS, reinterpret_cast<uint32_t*>(s));
+        tmem_ld32(tS + 32, reinterpret_cast<uint32_t*>(s) + 32);
+        tmem_ld32(tS + 64, reinterpret_cast<uint32_t*>(s) + 64);
+        tmem_ld32(tS + 96, reinterpret_cast<uint32_t*>(s) + 96);
+        tmem_wait_ld();
         const int b0 = wk.j * kTile;
         if (b0 + kTile - 1 > at0 + wk.sp.off || b0 + kTile > wk.sp.len) {
           const int lim = min(at0 + r + wk.sp.off, wk.sp.len - 1) - b0;  // last visible column
 #pragma unroll
           for (int c = 0; c < kTile; ++c)
-            if (c > lim) s[c] = 0xff800000u;  // -inf
+            if (c > lim) s[c] = -CUDART_INF_F;
         }
-        float mx0 = -CUDART_INF_F, mx1 = -CUDART_INF_F, mx2 = -CUDART_INF_F, mx3 = -CUDART_INF_F;
+        float mx0 = fmax3(s[0], s[1], s[2]), mx1 = fmax3(s[3], s[4], s[5]);
+        float mx2 = fmax3(s[6], s[7], s[8]), mx3 = fmax3(s[9], s[10], s[11]);
 #pragma unroll
-        for (int c = 0; c < kTile; c += 4) {
-          mx0 = fmaxf(mx0, __uint_as_float(s[c]));
-          mx1 = fmaxf(mx1, __uint_as_float(s[c + 1]));
-          mx2 = fmaxf(mx2, __uint_as_float(s[c + 2]));
-          mx3 = fmaxf(mx3, __uint_as_float(s[c + 3]));
+        for (int c = 12; c < 124; c += 8) {
+          mx0 = fmax3(mx0, s[c], s[c + 1]);
+          mx1 = fmax3(mx1, s[c + 2], s[c + 3]);
+          mx2 = fmax3(mx2, s[c + 4], s[c + 5]);
+          mx3 = fmax3(mx3, s[c + 6], s[c + 7]);
         }
+        mx0 = fmax3(mx0, s[124], s[125]);
+        mx1 = fmax3(mx1, s[126], s[127]);
         const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * p.scale_log2;
         const bool grow_max = mx > m_used + kRescaleThreshold;
         float alpha = 1.f;
         if (grow_max) {
           alpha = ex2(m_used - mx);  // 0 when nothing was visible so far
           m_used = mx;
-          l *= alpha;
+          l2.x *= alpha;
+          l2.y *= alpha;
         }
         if (cnt > 0 && __any_sync(0xffffffffu, grow_max)) {
           // S_t(b) complete implies PV_t(b-1) complete (issue order): O_t is stable here
@@ -360,28 +378,27 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tmem_st32(tO + c * 32, o);
           }
         }
-        const float m_eff = (m_used == -CUDART_INF_F) ? 0.f : m_used;
-        float l0 = 0.f, l1 = 0.f;
+        const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
+        const float2 nm2 = make_float2(neg_m, neg_m);
 #pragma unroll
         for (int c = 0; c < kTile / 32; ++c) {
           uint32_t pk[16];
 #pragma unroll
           for (int i = 0; i < 16; ++i) {
-            const float p0 = ex2(fmaf(__uint_as_float(s[c * 32 + 2 * i]), p.scale_log2, -m_eff));
-            const float p1 = ex2(fmaf(__uint_as_float(s[c * 32 + 2 * i + 1]), p.scale_log2, -m_eff));
-            l0 += p0;
-            l1 += p1;
-            pk[i] = pack_bf16(p0, p1);
+            const float2 x = fma2(make_float2(s[c * 32 + 2 * i], s[c * 32 + 2 * i + 1]), sc2, nm2);
+            const float2 e = make_float2(ex2(x.x), ex2(x.y));
+            l2 = add2(l2, e);
+            pk[i] = pack_bf16(e.x, e.y);
           }
           tmem_st16(tS + c * 16, pk);
         }
-        l += l0 + l1;
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(&p_full[t]);
         ++cnt;
       }
       // ------------------------------------ epilogue ------------------------------------
+      const float l = l2.x + l2.y;
       mbar_wait(&o_full[t], o_ph);
       o_ph ^= 1;
       tc_fence_after();
@@ -421,7 +438,7 @@ namespace bs {
 // Upload [header | items | spans | fill] into the workspace with one pageable-memory copy.
 bs_status_t upload_tables(const SchedTables& tb, void* ws, size_t ws_bytes, cudaStream_t st,
                           WsLayout* layout) {
-  const WsLayout L = ws_layout(tb.items.size(), tb.spans.size(), tb.fill.size());
+  const WsLayout L = ws_layout(tb.items.size(), tb.spans.size(), tb.groups.size(), tb.fill.size());
   BS_REQUIRE(ws != nullptr && ((uintptr_t)ws & 255) == 0, BS_ERR_WORKSPACE,
              "workspace is null or not 256-byte aligned");
   BS_REQUIRE(ws_bytes >= L.total, BS_ERR_WORKSPACE, "workspace too small: %zu < %zu bytes",
@@ -437,6 +454,10 @@ bs_status_t upload_tables(const SchedTables& tb, void* ws, size_t ws_bytes, cuda
   hd->n_items = (int32_t)tb.items.size();
   hd->n_spans = (int32_t)tb.spans.size();
   hd->n_fill = (int32_t)tb.fill.size();
+  hd->n_groups = (int32_t)tb.groups.size();
+  hd->n_units = tb.n_units;
+  if (!tb.groups.empty())
+    memcpy(blob.data() + L.groups_off, tb.groups.data(), tb.groups.size() * sizeof(Group));
   if (!tb.items.empty())
     memcpy(blob.data() + L.items_off, tb.items.data(), tb.items.size() * sizeof(Item));
   if (!tb.spans.empty())
@@ -489,7 +510,7 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
   cudaStream_t st = (cudaStream_t)stream;
   bs::SchedTables tb;
   rc = bs::build_fwd_tables(segs, n_segs, shape->q_rows, shape->kv_rows, out_row_begin, out_row_end,
-                            &tb);
+                            shape->n_q_heads, &tb);
   if (rc != BS_OK) return rc;
   bs::WsLayout L;
   rc = bs::upload_tables(tb, ws, ws_bytes, st, &L);
@@ -514,10 +535,7 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
   if (rc != BS_OK) return rc;
 
   FwdParams p;
-  p.items = (const bs::Item*)(wsb + L.items_off);
-  p.spans = (const bs::Span*)(wsb + L.spans_off);
-  p.counter = (int32_t*)wsb;
-  p.n_items = (int32_t)tb.items.size();
+  p.sv = bs::make_sched_view(wsb, L, tb, shape->n_q_heads);
   p.n_q_heads = shape->n_q_heads;
   p.group = shape->n_q_heads / shape->n_kv_heads;
   p.q_rows = shape->q_rows;
@@ -527,8 +545,7 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
   p.LSE = LSE;
   p.o_row_stride = shape->q_row_stride;
   p.lse_head_stride = shape->lse_head_stride;
-  const int64_t work = (int64_t)p.n_items * p.n_q_heads;
-  const int grid = (int)(work < bs::sm_count() ? work : bs::sm_count());
+  const int grid = tb.n_units < bs::sm_count() ? tb.n_units : bs::sm_count();
   if (D == 128) {
     BS_CUDA(cudaFuncSetAttribute(attn_fwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  FwdSmem<128>::kAlloc));

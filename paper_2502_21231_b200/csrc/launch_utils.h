@@ -32,3 +32,19 @@ bs_status_t upload_tables(const SchedTables& tb, void* ws, size_t ws_bytes, cuda
                           WsLayout* layout);
 int sm_count();
 }  // namespace bs
+
+#include "sched.cuh"
+namespace bs {
+inline SchedView make_sched_view(uint8_t* ws, const WsLayout& L, const SchedTables& tb,
+                                 int32_t n_heads) {
+  SchedView sv;
+  sv.counter = reinterpret_cast<int32_t*>(ws);
+  sv.items = reinterpret_cast<const Item*>(ws + L.items_off);
+  sv.spans = reinterpret_cast<const Span*>(ws + L.spans_off);
+  sv.groups = reinterpret_cast<const Group*>(ws + L.groups_off);
+  sv.n_groups = (int32_t)tb.groups.size();
+  sv.n_units = tb.n_units;
+  sv.n_heads = n_heads;
+  return sv;
+}
+}  // namespace bs

@@ -1,0 +1,83 @@
+// sched.cuh — device side of the persistent tile scheduler: one warp of the CTA
+// pulls unit indices from the global atomic cursor and hands them to the other warps through a
+// two-slot shared-memory ring, so every role of a warp-specialised kernel walks the same units.
+// The cursor order is the host's longest-first / locality order (worklist.h).
+#pragma once
+#include "ptx.cuh"
+#include "worklist.h"
+
+namespace bs {
+
+struct SchedView {  // device pointers into the uploaded workspace
+  int32_t* counter;
+  const Item* items;
+  const Span* spans;
+  const Group* groups;
+  int32_t n_groups, n_units, n_heads;
+};
+
+struct Unit {
+  Item item;
+  int32_t head;
+};
+
+// unit index -> (item, head): binary search of the group, then head-major inside the group.
+__device__ __forceinline__ Unit decode_unit(const SchedView& sv, int32_t w) {
+  int lo = 0, hi = sv.n_groups - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (sv.groups[mid].unit_begin <= w) lo = mid; else hi = mid - 1;
+  }
+  const Group g = sv.groups[lo];
+  const int local = w - g.unit_begin;
+  Unit u;
+  u.head = local / g.n_items;
+  u.item = sv.items[g.item_begin + local % g.n_items];
+  return u;
+}
+
+constexpr int kSchedSlots = 2;
+
+struct SchedRing {  // lives in shared memory
+  uint64_t full[kSchedSlots], empty[kSchedSlots];
+  int32_t unit[kSchedSlots];
+};
+
+// n_consumers = threads that call UnitConsumer::next()
+__device__ __forceinline__ void sched_ring_init(SchedRing* r, uint32_t n_consumers) {
+  for (int i = 0; i < kSchedSlots; ++i) {
+    ptx::mbar_init(&r->full[i], 1);
+    ptx::mbar_init(&r->empty[i], n_consumers);
+  }
+}
+
+struct UnitProducer {  // one thread
+  SchedRing* r;
+  uint32_t n = 0;
+  // Returns the next unit index of this CTA, or -1 when the cursor ran out (also published).
+  __device__ __forceinline__ int32_t next(const SchedView& sv) {
+    int32_t w = atomicAdd(sv.counter, 1);
+    if (w >= sv.n_units) w = -1;
+    const uint32_t slot = n % kSchedSlots, ph = (n / kSchedSlots) & 1;
+    ptx::mbar_wait(&r->empty[slot], ph ^ 1);
+    r->unit[slot] = w;
+    ptx::mbar_arrive(&r->full[slot]);
+    ++n;
+    return w;
+  }
+};
+
+struct UnitConsumer {  // every consuming thread
+  SchedRing* r;
+  uint32_t n = 0;
+  __device__ __forceinline__ int32_t next() {
+    const uint32_t slot = n % kSchedSlots, ph = (n / kSchedSlots) & 1;
+    ptx::mbar_wait(&r->full[slot], ph);
+    const int32_t w = r->unit[slot];
+    ptx::mbar_arrive(&r->empty[slot]);
+    ++n;
+    return w;
+  }
+};
+
+}  // namespace bs

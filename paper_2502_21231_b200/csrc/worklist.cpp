@@ -46,11 +46,12 @@ bs_status_t check_seg(const bs_seg_t& g, int i, int32_t q_rows, int32_t kv_rows)
 }
 }  // namespace
 
-WsLayout ws_layout(size_t n_items, size_t n_spans, size_t n_fill) {
+WsLayout ws_layout(size_t n_items, size_t n_spans, size_t n_groups, size_t n_fill) {
   WsLayout L;
   L.items_off = sizeof(SchedHeader);
   L.spans_off = align256(L.items_off + n_items * sizeof(Item));
-  L.fill_off = align256(L.spans_off + n_spans * sizeof(Span));
+  L.groups_off = align256(L.spans_off + n_spans * sizeof(Span));
+  L.fill_off = align256(L.groups_off + n_groups * sizeof(Group));
   L.total = align256(L.fill_off + n_fill * sizeof(RowRange));
   return L;
 }
@@ -59,12 +60,49 @@ size_t ws_upper_bound(int64_t rows, int32_t n_segs, bool bwd) {
   // items: every distinct range of length L yields ceil(L / tile) <= L / tile + 1 items
   const int64_t tile = bwd ? kTile : 2 * kTile;
   const size_t n_items = (size_t)(rows / tile + n_segs + 1);
-  return ws_layout(n_items, (size_t)n_segs, (size_t)n_segs + 1).total;
+  return ws_layout(n_items, (size_t)n_segs, (size_t)n_segs, (size_t)n_segs + 1).total;
 }
 
+namespace {
+// Order the groups by total cost (descending), the items of a group by cost (descending), and
+// number the units: group-major, then head, then item.
+bs_status_t finish_groups(std::vector<std::pair<int32_t, int32_t>>& group_items, int32_t n_heads,
+                          SchedTables* out) {
+  struct G {
+    int32_t begin, n;
+    int64_t cost;
+  };
+  std::vector<G> gs;
+  for (auto& gi : group_items) {
+    int64_t c = 0;
+    for (int32_t i = gi.first; i < gi.first + gi.second; ++i) c += out->items[i].cost;
+    gs.push_back({gi.first, gi.second, c});
+  }
+  std::stable_sort(gs.begin(), gs.end(), [](const G& a, const G& b) { return a.cost > b.cost; });
+  std::vector<Item> sorted;
+  sorted.reserve(out->items.size());
+  int64_t units = 0;
+  for (const G& g : gs) {
+    const int32_t begin = (int32_t)sorted.size();
+    sorted.insert(sorted.end(), out->items.begin() + g.begin, out->items.begin() + g.begin + g.n);
+    std::stable_sort(sorted.begin() + begin, sorted.end(),
+                     [](const Item& a, const Item& b) { return a.cost > b.cost; });
+    BS_REQUIRE(units + (int64_t)g.n * n_heads <= INT32_MAX, BS_ERR_INVALID_ARG,
+               "too many work units for one call");
+    out->groups.push_back({begin, g.n, (int32_t)units, 0});
+    units += (int64_t)g.n * n_heads;
+  }
+  out->items.swap(sorted);
+  out->n_units = (int32_t)units;
+  return BS_OK;
+}
+}  // namespace
+
 bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_rows, int32_t kv_rows,
-                             int32_t out_begin, int32_t out_end, SchedTables* out) {
+                             int32_t out_begin, int32_t out_end, int32_t n_heads,
+                             SchedTables* out) {
   try {
+    std::vector<std::pair<int32_t, int32_t>> group_items;
     std::vector<int32_t> order(n_segs);
     for (int32_t i = 0; i < n_segs; ++i) {
       bs_status_t rc = check_seg(segs[i], i, q_rows, kv_rows);
@@ -92,6 +130,7 @@ bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
       }
       ranges.push_back({g0.q_begin, g0.q_end});
       const int32_t q_len = g0.q_end - g0.q_begin;
+      group_items.push_back({(int32_t)out->items.size(), ceil_div(q_len, 2 * kTile)});
       for (int32_t a0 = 0; a0 < q_len; a0 += 2 * kTile) {
         Item it{};
         it.row0 = g0.q_begin + a0;
@@ -114,8 +153,8 @@ bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
       }
       i = j;
     }
-    std::stable_sort(out->items.begin(), out->items.end(),
-                     [](const Item& a, const Item& b) { return a.cost > b.cost; });
+    bs_status_t rc = finish_groups(group_items, n_heads, out);
+    if (rc != BS_OK) return rc;
     std::sort(ranges.begin(), ranges.end());
     return gaps_of(ranges, out_begin, out_end, "query", out);
   } catch (const std::bad_alloc&) {
@@ -124,8 +163,9 @@ bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
 }
 
 bs_status_t build_bwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_rows, int32_t kv_rows,
-                             SchedTables* out) {
+                             int32_t n_heads, SchedTables* out) {
   try {
+    std::vector<std::pair<int32_t, int32_t>> group_items;
     std::vector<int32_t> order(n_segs);
     for (int32_t i = 0; i < n_segs; ++i) {
       bs_status_t rc = check_seg(segs[i], i, q_rows, kv_rows);
@@ -149,6 +189,7 @@ bs_status_t build_bwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
       }
       ranges.push_back({g0.k_begin, g0.k_end});
       const int32_t k_len = g0.k_end - g0.k_begin;
+      group_items.push_back({(int32_t)out->items.size(), ceil_div(k_len, kTile)});
       for (int32_t b0 = 0; b0 < k_len; b0 += kTile) {
         Item it{};
         it.row0 = g0.k_begin + b0;
@@ -168,8 +209,8 @@ bs_status_t build_bwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
       }
       i = j;
     }
-    std::stable_sort(out->items.begin(), out->items.end(),
-                     [](const Item& a, const Item& b) { return a.cost > b.cost; });
+    bs_status_t rc = finish_groups(group_items, n_heads, out);
+    if (rc != BS_OK) return rc;
     std::sort(ranges.begin(), ranges.end());
     return gaps_of(ranges, 0, kv_rows, "key", out);
   } catch (const std::bad_alloc&) {

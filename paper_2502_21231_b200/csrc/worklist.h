@@ -1,7 +1,12 @@
 // worklist.h — work-item tables of the attention kernels (host-built, uploaded into the caller's
 // workspace).  This is the single-device analogue of the paper's balance scheduler (Alg. 2,
-// sort by cost descending, keep every worker equally loaded): items are ordered
-// longest-first and pulled by persistent CTAs.
+// sort by cost descending, always feed the least-loaded worker): work units are
+// ordered longest-first and pulled by persistent CTAs from one atomic cursor.
+//
+// Unit order (what the cursor walks): groups (= distinct ranges, most expensive first) x heads x
+// the group's items (most expensive first).  All CTAs therefore work on a handful of (range, head)
+// pairs at any time, whose K/V (forward) resp. Q/dO/dQ_acc (backward) rows stay in L2 while every
+// tile of the pair is processed; the cheapest units of the cheapest range come last (short tail).
 //
 // Forward item  = up to 256 consecutive query rows (two 128-row MMA tiles) of one distinct query
 //                 range; its spans are the key ranges of every segment on that query range
@@ -34,37 +39,47 @@ struct Item {
   int32_t cost;        // 128x128 blocks the item visits per head
   int32_t pad[2];
 };
+struct Group {           // the items of one distinct range; units = n_items x heads
+  int32_t item_begin;    // first item in the item table
+  int32_t n_items;
+  int32_t unit_begin;    // first unit index of the group
+  int32_t pad;
+};
 struct RowRange {
   int32_t begin, end;
 };
 struct SchedHeader {  // first 256 bytes of the workspace
   int32_t counter;    // dynamic scheduler cursor (zeroed by the upload)
   int32_t n_items, n_spans, n_fill;
-  int32_t pad[60];
+  int32_t n_groups, n_units;
+  int32_t pad[58];
 };
 static_assert(sizeof(SchedHeader) == 256, "header size");
-static_assert(sizeof(Item) == 32 && sizeof(Span) == 16, "table element sizes");
+static_assert(sizeof(Item) == 32 && sizeof(Span) == 16 && sizeof(Group) == 16, "table element sizes");
 
 struct SchedTables {
-  std::vector<Item> items;     // sorted by cost, descending
+  std::vector<Item> items;     // grouped by range; inside a group sorted by cost, descending
   std::vector<Span> spans;
+  std::vector<Group> groups;   // sorted by total cost, descending
+  int32_t n_units = 0;         // sum over groups of n_items x heads
   std::vector<RowRange> fill;  // rows of the output range covered by no item
   int64_t max_fill_rows = 0;
 };
 
-// Workspace layout: [SchedHeader][items][spans][fill ranges], each 256-byte aligned.
+// Workspace layout: [SchedHeader][items][spans][groups][fill ranges], each 256-byte aligned.
 struct WsLayout {
-  size_t items_off, spans_off, fill_off, total;
+  size_t items_off, spans_off, groups_off, fill_off, total;
 };
-WsLayout ws_layout(size_t n_items, size_t n_spans, size_t n_fill);
+WsLayout ws_layout(size_t n_items, size_t n_spans, size_t n_groups, size_t n_fill);
 // Upper bounds used by bs_attn_workspace_bytes (no segment list yet).
 size_t ws_upper_bound(int64_t rows, int32_t n_segs, bool bwd);
 
 // Forward: group segments by query range; rows [out_begin,out_end) not covered go to `fill`.
+// n_heads = heads the kernel multiplies the item list by (Hq forward, Hkv backward).
 bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_rows, int32_t kv_rows,
-                             int32_t out_begin, int32_t out_end, SchedTables* out);
+                             int32_t out_begin, int32_t out_end, int32_t n_heads, SchedTables* out);
 // Backward: group segments by key range; all kv_rows rows not covered go to `fill`.
 bs_status_t build_bwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_rows, int32_t kv_rows,
-                             SchedTables* out);
+                             int32_t n_heads, SchedTables* out);
 
 }  // namespace bs
