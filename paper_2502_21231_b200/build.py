@@ -18,7 +18,8 @@ ROOT = os.path.dirname(HERE)
 SO = os.path.join(CSRC, "libbytescale_attn.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+         "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC] + \
+    os.environ.get("BS_NVCC_EXTRA", "").split()  # e.g. -DBS_FWD_EMU=0 for kernel experiments
 
 
 def sources():

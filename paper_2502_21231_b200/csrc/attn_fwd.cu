@@ -4,13 +4,13 @@
 // Kernel shape (one persistent CTA per SM, 384 threads, registers re-split by setmaxnreg):
 //   warps 0-3  softmax warpgroup of Q tile 0   (thread r <-> row r of the 128-row tile)
 //   warps 4-7  softmax warpgroup of Q tile 1
-//   warp  8    MMA issuer (one elected lane): tcgen05.mma, accumulators in TMEM
-//   warp  9    TMA producer: Q per item and tile, K/V blocks through a 4-stage smem ring
+//   warps 8,10 MMA issuers of Q tile 0 / 1 (one lane each): tcgen05.mma, accumulators in TMEM
+//   warp  9    TMA producer + scheduler: Q per unit and tile, K/V blocks through a 4-stage ring
 // A work item is (up to 256 query rows = two 128-row tiles of one query range, one query head).
-// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,256+D) O1 [384,384+D); P (bf16) overwrites
-// the first 64 columns of its S.  Per KV block the tensor pipe runs, in issue order,
-//   PV0(b) S0(b+1) PV1(b) S1(b+1)
-// so that the softmax of one tile overlaps the MMAs of the other.  Softmax is fp32 with exp2,
+// TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,256+D) O1 [384,384+D); P (bf16) of 16 keys
+// overwrites the first 8 of the 16 S columns of those keys.  Per tile the chain is S(b) -> softmax -> P(b) -> PV(b), S(b+1);
+// the two tiles run this chain independently, so the softmax of one overlaps the MMAs of the
+// other, and P is handed over in two halves so that PV starts under the second half's exponentials.  Softmax is fp32 with exp2,
 // a lazily updated running max (rescale of O only when the max grew by more than 2^8) and the
 // row sum kept in fp32; O is normalised and written as bf16 with LSE = m ln2 + ln l at the end.
 #include <cuda_bf16.h>
@@ -28,11 +28,43 @@ namespace {
 using namespace bs;
 using namespace bs::ptx;
 
-constexpr int kFwdThreads = 384;      // 2 softmax warpgroups + 1 auxiliary warpgroup (MMA, TMA)
-constexpr int kRegsSoftmax = 208;     // setmaxnreg budgets: 256 * 208 + 128 * 88 = 384 * 168
-constexpr int kRegsAux = 88;
+constexpr int kFwdThreads = 640;      // 4 softmax warpgroups + 1 auxiliary warpgroup (MMA, TMA)
+constexpr int kMmaWarp0 = 16, kTmaWarp = 17;  // warps 16 / 18 issue the MMAs of Q tile 0 / 1
+constexpr int kRegsSoftmax = 104;     // setmaxnreg: 512 * 104 + 128 * 96 = 65536 (compiled at 96)
 constexpr int kStages = 4;              // K/V ring depth (K and V blocks alternate in the ring)
 constexpr float kRescaleThreshold = 8.f;  // log2 units
+#ifndef BS_FWD_EMU
+#define BS_FWD_EMU 1
+#endif
+constexpr int kEmuOf4 = BS_FWD_EMU;  // of every 4 column pairs, this many take the FMA-pipe exp2
+
+// 2^x for x <= ~8 on the FMA pipe (the MUFU unit is co-critical with the tensor pipe, SURVEY.md
+// 7.2-3): round-to-nearest split x = n + f with the 1.5 * 2^23 trick, degree-3 minimax polynomial
+// of 2^f on [-0.5, 0.5] (relative error 7.5e-5, far below the bf16 rounding of P), n added into
+// the exponent field.  x is clamped at -125, so masked (-inf) scores give ~2^-125 instead of 0.
+__device__ __forceinline__ float2 ex2_fma2(float2 x) {
+  x.x = fmaxf(x.x, -125.f);
+  x.y = fmaxf(x.y, -125.f);
+  const float2 t = add2(x, make_float2(12582912.f, 12582912.f));
+  const float2 n = add2(t, make_float2(-12582912.f, -12582912.f));
+  const float2 f = add2(x, make_float2(-n.x, -n.y));
+  float2 q = fma2(f, make_float2(0.0551716685f, 0.0551716685f), make_float2(0.242611125f, 0.242611125f));
+  q = fma2(q, f, make_float2(0.693260968f, 0.693260968f));
+  q = fma2(q, f, make_float2(0.999928057f, 0.999928057f));
+  return make_float2(__int_as_float(__float_as_int(q.x) + (__float_as_int(t.x) << 23)),
+                     __int_as_float(__float_as_int(q.y) + (__float_as_int(t.y) << 23)));
+}
+
+#ifdef BS_FWD_TRACE
+// debug build only: per-event clock64() stamps of CTA 0 (role, event) x iteration
+__device__ long long g_fwd_trace[4][8][256];
+#define TRACE(role, ev, it)                                                    \
+  do {                                                                         \
+    if (blockIdx.x == 0 && (it) < 256) g_fwd_trace[role][ev][it] = clock64();  \
+  } while (0)
+#else
+#define TRACE(role, ev, it) do {} while (0)
+#endif
 
 struct FwdParams {
   SchedView sv;     // units = query items x n_q_heads
@@ -50,11 +82,13 @@ struct FwdSmem {
   static constexpr int kQOff = 0;                   // 2 Q tiles
   static constexpr int kKVOff = 2 * kTileBytes;     // kStages K/V tiles
   static constexpr int kBarOff = kKVOff + kStages * kTileBytes;
-  // barriers: q_full[2], q_empty[2], kv_full[S], kv_empty[S], s_full[2], p_full[2], o_full[2]
-  static constexpr int kNumBars = 4 + 2 * kStages + 6;
+  // barriers: q_full[2], q_empty[2], kv_full[S], kv_empty[S], s_full[2], p_full[2][2], o_full[2]
+  static constexpr int kNumBars = 4 + 2 * kStages + 8;
   static constexpr int kTmemSlotOff = kBarOff + kNumBars * 8;
   static constexpr int kSchedOff = kTmemSlotOff + 8;  // SchedRing of the dynamic scheduler
-  static constexpr int kBytes = kSchedOff + 64;
+  static constexpr int kXchOff = kSchedOff + 64;      // row max [2 tiles][2][2][128], row sum [2][2][128]
+  static constexpr int kLockOff = kXchOff + 6144;     // turn lock of the two MMA issuers
+  static constexpr int kBytes = kLockOff + 16;
   static constexpr int kAlloc = kBytes + 1024;  // slack to align the base to 1024 B
 };
 
@@ -68,17 +102,26 @@ __device__ __forceinline__ int span_blocks(int at0, int rows, const Span& sp) {
 
 
 // Walks the 128-key blocks of an item in (span, block) order.  A block is visited if either Q
-// tile has a visible pair in it; tile t takes part in the block iff active(t).
-struct Walker {
+// tile has a visible pair in it; tile t takes part in the block iff active(t).  (Scalar members
+// only: arrays indexed by the runtime tile number would live in local memory.)
+template <bool kUniform>
+struct WalkerT {
   const Span* spans;
-  int n_spans, s, j, nb[2], at0[2], rows[2];
+  int n_spans, s, j, nb0, nb1, at0_1, rows0, rows1;
   Span sp;
+  __device__ __forceinline__ int at0(int t) const { return t ? at0_1 : at0_1 - kTile; }
+  __device__ __forceinline__ int rows(int t) const { return t ? rows1 : rows0; }
   __device__ __forceinline__ void load_span() {
     while (s < n_spans) {
       sp = spans[s];
-      nb[0] = span_blocks(at0[0], rows[0], sp);
-      nb[1] = span_blocks(at0[1], rows[1], sp);
-      if (max(nb[0], nb[1]) > 0) break;
+      if (kUniform) {  // converged warp, same span in every lane
+        sp.begin = warp_uniform(sp.begin);
+        sp.len = warp_uniform(sp.len);
+        sp.off = warp_uniform(sp.off);
+      }
+      nb0 = span_blocks(at0_1 - kTile, rows0, sp);
+      nb1 = span_blocks(at0_1, rows1, sp);
+      if (max(nb0, nb1) > 0) break;
       ++s;
     }
     j = 0;
@@ -86,17 +129,16 @@ struct Walker {
   __device__ __forceinline__ void init(const Span* sp_table, const Item& it) {
     spans = sp_table + it.span_begin;
     n_spans = it.n_spans;
-    for (int t = 0; t < 2; ++t) {
-      at0[t] = it.local0 + t * kTile;
-      rows[t] = max(0, min(kTile, it.range_len - at0[t]));
-    }
+    at0_1 = it.local0 + kTile;
+    rows0 = max(0, min(kTile, it.range_len - it.local0));
+    rows1 = max(0, min(kTile, it.range_len - at0_1));
     s = 0;
     load_span();
   }
   __device__ __forceinline__ bool done() const { return s >= n_spans; }
-  __device__ __forceinline__ bool active(int t) const { return j < nb[t]; }
+  __device__ __forceinline__ bool active(int t) const { return j < (t ? nb1 : nb0); }
   __device__ __forceinline__ void next() {
-    if (++j >= max(nb[0], nb[1])) {
+    if (++j >= max(nb0, nb1)) {
       ++s;
       load_span();
     }
@@ -104,10 +146,11 @@ struct Walker {
   // total blocks tile t takes part in over the whole item
   __device__ __forceinline__ int total(int t) const {
     int n = 0;
-    for (int q = 0; q < n_spans; ++q) n += span_blocks(at0[t], rows[t], spans[q]);
-    return n;
+    for (int q = 0; q < n_spans; ++q) n += span_blocks(at0(t), rows(t), spans[q]);
+    return kUniform ? warp_uniform(n) : n;
   }
 };
+using Walker = WalkerT<false>;
 
 template <int D>
 __device__ __forceinline__ void issue_qk(uint32_t tmem_s, uint32_t q_addr, uint32_t k_addr) {
@@ -119,14 +162,17 @@ __device__ __forceinline__ void issue_qk(uint32_t tmem_s, uint32_t q_addr, uint3
             idesc, kk > 0);
   }
 }
+// O (+)= P V for keys [64 half, 64 half + 64) of the block
 template <int D>
-__device__ __forceinline__ void issue_pv(uint32_t tmem_o, uint32_t tmem_p, uint32_t v_addr,
-                                         bool accumulate) {
+__device__ __forceinline__ void issue_pv_half(uint32_t tmem_o, uint32_t tmem_p, uint32_t v_addr,
+                                              int half, bool accumulate) {
   constexpr uint32_t idesc = umma_idesc_bf16(kTile, D, 0, 1);  // B = V is MN-major (d contiguous)
 #pragma unroll
-  for (int kk = 0; kk < kTile / 16; ++kk) {
+  for (int k4 = 0; k4 < 4; ++k4) {
+    const int kk = half * 4 + k4;
     // 16 keys = 16 rows of 128 B; the second 64-wide d half (D = 128) is one box (16 KB) further
-    umma_ts(tmem_o, tmem_p + kk * 8, umma_desc_sw128(v_addr + kk * 2048, kTile * 128, 1024), idesc,
+    // P of keys [16 kk, 16 kk + 16) sits over the first 8 columns of its own 16 S columns
+    umma_ts(tmem_o, tmem_p + kk * 16, umma_desc_sw128(v_addr + kk * 2048, kTile * 128, 1024), idesc,
             accumulate || kk > 0);
   }
 }
@@ -159,40 +205,41 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint64_t* kv_full = bars + 4;
   uint64_t* kv_empty = bars + 4 + kStages;
   uint64_t* s_full = bars + 4 + 2 * kStages;
-  uint64_t* p_full = s_full + 2;
-  uint64_t* o_full = p_full + 2;
+  uint64_t* p_full = s_full + 2;  // [tile][half]
+  uint64_t* o_full = p_full + 4;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kTmemSlotOff);
   SchedRing* sched = reinterpret_cast<SchedRing*>(smem + L::kSchedOff);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
-  if (warp == 9 && lane == 0) {
-    sched_ring_init(sched, 2 * kTile + 1);  // consumers: 256 softmax threads + the MMA lane
+  if (warp == kTmaWarp && lane == 0) {
+    *reinterpret_cast<uint32_t*>(smem + L::kLockOff) = 0;
+    sched_ring_init(sched, 4 * kTile + 2);  // consumers: 512 softmax threads + 2 MMA lanes
     for (int t = 0; t < 2; ++t) {
       mbar_init(&q_full[t], 1);
       mbar_init(&q_empty[t], 1);
       mbar_init(&s_full[t], 1);
-      mbar_init(&p_full[t], kTile);
+      mbar_init(&p_full[2 * t], 4);  // one arrival per softmax warp
+      mbar_init(&p_full[2 * t + 1], 4);
       mbar_init(&o_full[t], 1);
     }
     for (int i = 0; i < kStages; ++i) {
       mbar_init(&kv_full[i], 1);
-      mbar_init(&kv_empty[i], 1);
+      mbar_init(&kv_empty[i], 2);  // both MMA issuers release a stage
     }
     fence_barrier_init();
     prefetch_tensormap(&tmQ);
     prefetch_tensormap(&tmK);
     prefetch_tensormap(&tmV);
   }
-  if (warp == 8) tmem_alloc<512>(tmem_slot);
+  if (warp == kMmaWarp0) tmem_alloc<512>(tmem_slot);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
   const uint32_t smem_q = smem_u32(smem + L::kQOff), smem_kv = smem_u32(smem + L::kKVOff);
 
-  if (warp >= 8) {
-    setmaxnreg_dec<kRegsAux>();
-    if (warp == 9 && lane == 0) {
+  if (warp >= kMmaWarp0) {
+    if (warp == kTmaWarp && lane == 0) {
       // ===================================== TMA producer =====================================
       uint32_t q_ph[2] = {0, 0};
       Ring ring;
@@ -230,39 +277,54 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           }
         }
       }
-    } else if (warp == 8 && lane == 0) {
-      // ====================================== MMA issuer ======================================
-      uint32_t q_ph[2] = {0, 0}, p_ph[2] = {0, 0};
+    } else if ((warp == kMmaWarp0 || warp == kMmaWarp0 + 2) && lane == 0) {
+      // ============================ MMA issuer of Q tile t = 0 / 1 ============================
+      // Each tile has its own issuing warp (one lane).
+      const int t = (warp - kMmaWarp0) >> 1;
+      const uint32_t tS = tmem + t * kTile, tO = tmem + 256 + t * kTile;
+      const uint32_t sQ = smem_q + t * L::kTileBytes;
+      uint32_t q_ph = 0, p_ph = 0;
+      uint32_t* turn = reinterpret_cast<uint32_t*>(smem + L::kLockOff);
+      int tr_it = 0;
       Ring ring;
       UnitConsumer cons{sched};
       int32_t w;
       while ((w = cons.next()) >= 0) {
         const Unit u = decode_unit(p.sv, w);
-        const Item& it = u.item;
         Walker cur;
-        cur.init(p.sv.spans, it);
+        cur.init(p.sv.spans, u.item);
         if (cur.done()) continue;
-        const int tot[2] = {cur.total(0), cur.total(1)};
-        int n_s[2] = {0, 0}, n_pv[2] = {0, 0};
-        // S_t = Q_t K^T of one block; the first one of an item waits for the tile's Q, the last
-        // one releases the tile's Q buffer to the producer (next item's Q streams in early)
-        auto issue_s = [&](int t, uint32_t k_stage) {
-          if (n_s[t] == 0) {
-            mbar_wait(&q_full[t], q_ph[t]);
-            q_ph[t] ^= 1;
+        const int tot = cur.total(t);
+        int n_s = 0, n_pv = 0;
+        auto wait_q = [&]() {  // never called with the turn lock held
+          if (n_s == 0) {
+            mbar_wait(&q_full[t], q_ph);
+            q_ph ^= 1;
             tc_fence_after();
           }
-          issue_qk<D>(tmem + t * kTile, smem_q + t * L::kTileBytes,
-                      smem_kv + k_stage * L::kTileBytes);
-          tc_commit(&s_full[t]);
-          if (++n_s[t] == tot[t]) tc_commit(&q_empty[t]);
         };
-        // prologue: S_t(0)
+        // S_t = Q_t K^T of one block; the last one of a unit releases the tile's Q buffer to the
+        // producer (the next unit's Q streams in early)
+        auto issue_s = [&](uint32_t k_stage) {
+          ++n_s;
+          {
+            issue_qk<D>(tS, sQ, smem_kv + k_stage * L::kTileBytes);
+            tc_commit(&s_full[t]);
+            if (n_s == tot) tc_commit(&q_empty[t]);
+          }
+        };
+        auto release = [&](uint32_t stage) {
+          tc_commit(&kv_empty[stage]);
+        };
+        // prologue: S_t(0).  Every ring stage is waited for and released by both issuers, also
+        // for blocks their tile takes no part in.
         mbar_wait(&kv_full[ring.stage], ring.phase);
         tc_fence_after();
-        for (int t = 0; t < 2; ++t)
-          if (cur.active(t)) issue_s(t, ring.stage);
-        tc_commit(&kv_empty[ring.stage]);
+        if (cur.active(t)) {
+          wait_q();
+          issue_s(ring.stage);
+        }
+        release(ring.stage);
         ring.advance();
         while (true) {
           Walker nxt = cur;
@@ -277,34 +339,58 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             ring.advance();
           }
           tc_fence_after();
-          for (int t = 0; t < 2; ++t) {
-            if (cur.active(t)) {
-              mbar_wait(&p_full[t], p_ph[t]);
-              p_ph[t] ^= 1;
-              tc_fence_after();
-              issue_pv<D>(tmem + 256 + t * kTile, tmem + t * kTile,
-                          smem_kv + v_stage * L::kTileBytes, n_pv[t] > 0);
-              if (++n_pv[t] == tot[t]) tc_commit(&o_full[t]);
-            }
-            if (has_next && nxt.active(t)) issue_s(t, k_stage);
+          if (cur.active(t)) {
+            mbar_wait(&p_full[2 * t], p_ph);      // the two column halves of P
+            mbar_wait(&p_full[2 * t + 1], p_ph);
+            p_ph ^= 1;
+            if (lane == 0) TRACE(2 + t, 0, tr_it);
+            tc_fence_after();
           }
-          tc_commit(&kv_empty[v_stage]);
+          if (has_next && nxt.active(t)) wait_q();
+          // The batch [PV_t(b), S_t(b+1)] is issued under the turn lock: batches of the two tiles
+          // enter the tensor pipe whole, one after the other, which keeps the tiles half a period
+          // apart (softmax of one under the MMAs of the other) instead of drifting into phase.
+          while (atom_cas_shared(turn, 0u, 1u) != 0u) __nanosleep(20);
+          if (lane == 0) TRACE(2 + t, 1, tr_it);
+          if (cur.active(t)) {
+            ++n_pv;
+            {
+              issue_pv_half<D>(tO, tS, smem_kv + v_stage * L::kTileBytes, 0, n_pv > 1);
+              issue_pv_half<D>(tO, tS, smem_kv + v_stage * L::kTileBytes, 1, true);
+              if (n_pv == tot) tc_commit(&o_full[t]);
+            }
+              if (lane == 0) TRACE(2 + t, 2, tr_it);
+          }
+          release(v_stage);
+          if (has_next) {
+            if (nxt.active(t)) issue_s(k_stage);
+            release(k_stage);
+          }
+          if (lane == 0) TRACE(2 + t, 3, tr_it);
+          st_release_shared(turn, 0u);
+          if (lane == 0) TRACE(2 + t, 4, tr_it);
+          ++tr_it;
           if (!has_next) break;
-          tc_commit(&kv_empty[k_stage]);
           cur = nxt;
         }
       }
     }
   } else {
     // ================================== softmax warpgroups ==================================
-    setmaxnreg_inc<kRegsSoftmax>();
-    const int t = warp >> 2;            // Q tile of this warpgroup
+    // Warpgroup g = warp / 4 works on Q tile t = g / 2, key columns [64 hf, 64 hf + 64) with
+    // hf = g % 2: two threads share a row (the row maximum and the row sum are exchanged through
+    // shared memory), which halves the latency of the S -> P step that the MMAs wait for.
+    // (no setmaxnreg: the kernel is compiled for 96 registers per thread, 640 * 96 = 61440)
+    const int t = warp >> 3, hf = (warp >> 2) & 1;
     const int r = threadIdx.x & 127;    // row of the tile owned by this thread
     const uint32_t lane_addr = uint32_t((warp & 3) * 32) << 16;
-    const uint32_t tS = tmem + lane_addr + t * kTile;        // S_t, and P_t over its first 64 cols
-    const uint32_t tO = tmem + lane_addr + 256 + t * kTile;  // O_t
+    const uint32_t tS = tmem + lane_addr + t * kTile + hf * 64;         // this half of S_t
+    const uint32_t tO = tmem + lane_addr + 256 + t * kTile + hf * (D / 2);  // this half of O_t
+    float* xch_m = reinterpret_cast<float*>(smem + L::kXchOff) + t * 512 + r;  // [parity][half][row]
+    float* xch_l = reinterpret_cast<float*>(smem + L::kXchOff) + 1024 + t * 256 + r;  // [half][row]
     const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
     uint32_t s_ph = 0, o_ph = 0;
+    int tr_it = 0;
     UnitConsumer cons{sched};
     int32_t w;
     while ((w = cons.next()) >= 0) {
@@ -313,15 +399,15 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const int h = u.head;
       Walker wk;
       wk.init(p.sv.spans, it);
-      const int at0 = wk.at0[t];
-      const bool valid = r < wk.rows[t];
+      const int at0 = wk.at0(t);
+      const bool valid = r < wk.rows(t);
       const int64_t grow = (int64_t)it.row0 + t * kTile + r;
-      __nv_bfloat16* o_ptr = p.O + grow * p.o_row_stride + (int64_t)h * D;
+      __nv_bfloat16* o_ptr = p.O + grow * p.o_row_stride + (int64_t)h * D + hf * (D / 2);
       const int tot = wk.total(t);
       if (tot == 0) {  // no key of this call is visible to any row of the tile
         if (valid) {
-          for (int c = 0; c < D / 8; ++c) reinterpret_cast<uint4*>(o_ptr)[c] = make_uint4(0, 0, 0, 0);
-          p.LSE[(int64_t)h * p.lse_head_stride + grow] = -CUDART_INF_F;
+          for (int c = 0; c < D / 16; ++c) reinterpret_cast<uint4*>(o_ptr)[c] = make_uint4(0, 0, 0, 0);
+          if (hf == 0) p.LSE[(int64_t)h * p.lse_head_stride + grow] = -CUDART_INF_F;
         }
         continue;
       }
@@ -332,32 +418,52 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (!wk.active(t)) continue;
         mbar_wait(&s_full[t], s_ph);
         s_ph ^= 1;
+        if (r == 0) TRACE(t, 0, tr_it);
         tc_fence_after();
-        float s[kTile];
-        tmem_ld32(tS, reinterpret_cast<uint32_t*>(s));
-        tmem_ld32(tS + 32, reinterpret_cast<uint32_t*>(s) + 32);
-        tmem_ld32(tS + 64, reinterpret_cast<uint32_t*>(s) + 64);
-        tmem_ld32(tS + 96, reinterpret_cast<uint32_t*>(s) + 96);
-        tmem_wait_ld();
+        // Two passes over this thread's 64 columns in chunks of 16, double-buffered in A / B so
+        // that the TMEM load of the next chunk runs under the arithmetic of the current one.
+        // Pass 1: row maximum.  Pass 2 (chunks 3, 0, 1, 2; chunk 3 is still in B): P = 2^(S c - m),
+        // packed to bf16 and written over the chunk's own first 8 columns.
         const int b0 = wk.j * kTile;
-        if (b0 + kTile - 1 > at0 + wk.sp.off || b0 + kTile > wk.sp.len) {
-          const int lim = min(at0 + r + wk.sp.off, wk.sp.len - 1) - b0;  // last visible column
+        const bool edge = b0 + kTile - 1 > at0 + wk.sp.off || b0 + kTile > wk.sp.len;
+        // last visible column of this row relative to this thread's first column (>= 63: all)
+        const int lim = edge ? min(at0 + r + wk.sp.off, wk.sp.len - 1) - b0 - hf * 64 : 64;
+        float A[16], B[16];
+        auto mask16 = [&](float* v, int lim_k) {
 #pragma unroll
-          for (int c = 0; c < kTile; ++c)
-            if (c > lim) s[c] = -CUDART_INF_F;
-        }
-        float mx0 = fmax3(s[0], s[1], s[2]), mx1 = fmax3(s[3], s[4], s[5]);
-        float mx2 = fmax3(s[6], s[7], s[8]), mx3 = fmax3(s[9], s[10], s[11]);
+          for (int c = 0; c < 16; ++c)
+            if (c > lim_k) v[c] = -CUDART_INF_F;
+        };
+        float mx0 = -CUDART_INF_F, mx1 = -CUDART_INF_F;
+        auto max16 = [&](const float* v) {
 #pragma unroll
-        for (int c = 12; c < 124; c += 8) {
-          mx0 = fmax3(mx0, s[c], s[c + 1]);
-          mx1 = fmax3(mx1, s[c + 2], s[c + 3]);
-          mx2 = fmax3(mx2, s[c + 4], s[c + 5]);
-          mx3 = fmax3(mx3, s[c + 6], s[c + 7]);
-        }
-        mx0 = fmax3(mx0, s[124], s[125]);
-        mx1 = fmax3(mx1, s[126], s[127]);
-        const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * p.scale_log2;
+          for (int c = 0; c < 16; c += 4) {
+            mx0 = fmax3(mx0, v[c], v[c + 1]);
+            mx1 = fmax3(mx1, v[c + 2], v[c + 3]);
+          }
+        };
+        tmem_ld16(tS, reinterpret_cast<uint32_t*>(A));
+        tmem_wait_ld();
+        tmem_ld16(tS + 16, reinterpret_cast<uint32_t*>(B));
+        if (lim < 15) mask16(A, lim);
+        max16(A);
+        tmem_wait_ld();
+        tmem_ld16(tS + 32, reinterpret_cast<uint32_t*>(A));
+        if (lim < 31) mask16(B, lim - 16);
+        max16(B);
+        tmem_wait_ld();
+        tmem_ld16(tS + 48, reinterpret_cast<uint32_t*>(B));
+        if (lim < 47) mask16(A, lim - 32);
+        max16(A);
+        tmem_wait_ld();
+        if (lim < 63) mask16(B, lim - 48);
+        max16(B);
+        if (r == 0) TRACE(t, 1, tr_it);
+        const float mx_half = fmaxf(mx0, mx1);
+        // exchange the half-row maxima (slots alternate with the block parity; one barrier/block)
+        xch_m[(cnt & 1) * 256 + hf * 128] = mx_half;
+        bar_sync(1 + t, 2 * kTile);
+        const float mx = fmaxf(mx_half, xch_m[(cnt & 1) * 256 + (hf ^ 1) * 128]) * p.scale_log2;
         const bool grow_max = mx > m_used + kRescaleThreshold;
         float alpha = 1.f;
         if (grow_max) {
@@ -368,59 +474,84 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
         if (cnt > 0 && __any_sync(0xffffffffu, grow_max)) {
           // S_t(b) complete implies PV_t(b-1) complete (issue order): O_t is stable here
-#pragma unroll
+#pragma unroll 1
           for (int c = 0; c < D / 32; ++c) {
-            uint32_t o[32];
-            tmem_ld32(tO + c * 32, o);
+            uint32_t o[16];
+            tmem_ld16(tO + c * 16, o);
             tmem_wait_ld();
 #pragma unroll
-            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-            tmem_st32(tO + c * 32, o);
+            for (int i = 0; i < 16; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+            tmem_st16(tO + c * 16, o);
           }
         }
+        if (r == 0) TRACE(t, 2, tr_it);
         const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
         const float2 nm2 = make_float2(neg_m, neg_m);
+        auto exp16 = [&](const float* v, int k) {
+          uint32_t pk[8];
 #pragma unroll
-        for (int c = 0; c < kTile / 32; ++c) {
-          uint32_t pk[16];
-#pragma unroll
-          for (int i = 0; i < 16; ++i) {
-            const float2 x = fma2(make_float2(s[c * 32 + 2 * i], s[c * 32 + 2 * i + 1]), sc2, nm2);
-            const float2 e = make_float2(ex2(x.x), ex2(x.y));
+          for (int i = 0; i < 8; ++i) {
+            const float2 x = fma2(make_float2(v[2 * i], v[2 * i + 1]), sc2, nm2);
+            const float2 e = (i & 3) < kEmuOf4 ? ex2_fma2(x) : make_float2(ex2(x.x), ex2(x.y));
             l2 = add2(l2, e);
             pk[i] = pack_bf16(e.x, e.y);
           }
-          tmem_st16(tS + c * 16, pk);
-        }
+          tmem_st8(tS + 16 * k, pk);
+        };
+#ifndef BS_FWD_NORELOAD
+#define RELOAD(addr, dst) tmem_ld16(addr, reinterpret_cast<uint32_t*>(dst))
+#else
+#define RELOAD(addr, dst) do {} while (0)  /* experiment only: wrong results */
+#endif
+        RELOAD(tS, A);
+        exp16(B, 3);
+        tmem_wait_ld();
+        RELOAD(tS + 16, B);
+        if (lim < 15) mask16(A, lim);
+        exp16(A, 0);
+        tmem_wait_ld();
+        RELOAD(tS + 32, A);
+        if (lim < 31) mask16(B, lim - 16);
+        exp16(B, 1);
+        tmem_wait_ld();
+        if (lim < 47) mask16(A, lim - 32);
+        exp16(A, 2);
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(&p_full[t]);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&p_full[2 * t + hf]);
+        if (r == 0) TRACE(t, 3 + hf, tr_it);
+        ++tr_it;
         ++cnt;
       }
       // ------------------------------------ epilogue ------------------------------------
-      const float l = l2.x + l2.y;
+      // rows that saw no key: the emulated exp2 leaves ~2^-125 per masked score in l
+      const float l_half = m_used == -CUDART_INF_F ? 0.f : l2.x + l2.y;
+      xch_l[hf * 128] = l_half;
+      bar_sync(1 + t, 2 * kTile);
+      const float l = l_half + xch_l[(hf ^ 1) * 128];
       mbar_wait(&o_full[t], o_ph);
       o_ph ^= 1;
       tc_fence_after();
       const float inv_l = l > 0.f ? 1.f / l : 0.f;
 #pragma unroll
       for (int c = 0; c < D / 32; ++c) {
-        uint32_t o[32];
-        tmem_ld32(tO + c * 32, o);
+        uint32_t o[16];
+        tmem_ld16(tO + c * 16, o);
         tmem_wait_ld();
         if (valid) {
 #pragma unroll
-          for (int v = 0; v < 4; ++v) {
+          for (int v = 0; v < 2; ++v) {
             uint4 pk;
             pk.x = pack_bf16(__uint_as_float(o[8 * v + 0]) * inv_l, __uint_as_float(o[8 * v + 1]) * inv_l);
             pk.y = pack_bf16(__uint_as_float(o[8 * v + 2]) * inv_l, __uint_as_float(o[8 * v + 3]) * inv_l);
             pk.z = pack_bf16(__uint_as_float(o[8 * v + 4]) * inv_l, __uint_as_float(o[8 * v + 5]) * inv_l);
             pk.w = pack_bf16(__uint_as_float(o[8 * v + 6]) * inv_l, __uint_as_float(o[8 * v + 7]) * inv_l);
-            reinterpret_cast<uint4*>(o_ptr)[c * 4 + v] = pk;
+            reinterpret_cast<uint4*>(o_ptr)[c * 2 + v] = pk;
           }
         }
       }
-      if (valid)
+      if (valid && hf == 0)
         p.LSE[(int64_t)h * p.lse_head_stride + grow] =
             l > 0.f ? m_used * 0.69314718055994531f + __logf(l) : -CUDART_INF_F;
       tc_fence_before();
@@ -428,7 +559,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 8) tmem_dealloc<512>(tmem);
+  if (warp == kMmaWarp0) tmem_dealloc<512>(tmem);
 }
 
 }  // namespace
@@ -481,6 +612,12 @@ int sm_count() {
 }
 
 }  // namespace bs
+
+#ifdef BS_FWD_TRACE
+extern "C" int bs_debug_fwd_trace(long long* host_out) {
+  return (int)cudaMemcpyFromSymbol(host_out, g_fwd_trace, sizeof(g_fwd_trace));
+}
+#endif
 
 extern "C" {
 

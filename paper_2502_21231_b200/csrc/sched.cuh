@@ -67,6 +67,13 @@ struct UnitProducer {  // one thread
   }
 };
 
+// Tell the compiler that a value is the same in every lane of a converged warp (it then keeps
+// it, and what is computed from it, in uniform registers - e.g. the tcgen05.mma descriptors).
+template <class T>
+__device__ __forceinline__ T warp_uniform(T v) {
+  return __shfl_sync(0xffffffffu, v, 0);
+}
+
 struct UnitConsumer {  // every consuming thread
   SchedRing* r;
   uint32_t n = 0;
@@ -78,6 +85,28 @@ struct UnitConsumer {  // every consuming thread
     ++n;
     return w;
   }
+  // Whole converged warp consumes as ONE consumer (one arrival on the empty barrier).
+  __device__ __forceinline__ int32_t next_warp() {
+    const uint32_t slot = n % kSchedSlots, ph = (n / kSchedSlots) & 1;
+    ptx::mbar_wait_warp(&r->full[slot], ph);
+    const int32_t w = warp_uniform(r->unit[slot]);
+    __syncwarp();
+    if (ptx::elect_one()) ptx::mbar_arrive(&r->empty[slot]);
+    ++n;
+    return w;
+  }
 };
+
+// decode_unit for a converged warp: every lane loads the same words; the fields come back uniform.
+__device__ __forceinline__ Unit decode_unit_warp(const SchedView& sv, int32_t w) {
+  Unit u = decode_unit(sv, w);
+  u.head = warp_uniform(u.head);
+  u.item.row0 = warp_uniform(u.item.row0);
+  u.item.local0 = warp_uniform(u.item.local0);
+  u.item.range_len = warp_uniform(u.item.range_len);
+  u.item.span_begin = warp_uniform(u.item.span_begin);
+  u.item.n_spans = warp_uniform(u.item.n_spans);
+  return u;
+}
 
 }  // namespace bs
