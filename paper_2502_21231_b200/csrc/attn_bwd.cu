@@ -36,6 +36,17 @@ using namespace bs::ptx;
 constexpr int kBwdThreads = 384;
 constexpr int kComputeThreads = 256;
 
+#ifdef BS_BWD_TRACE
+// debug build only: clock64() stamps of CTA 0: [role][event][iteration]
+__device__ long long g_bwd_trace[3][10][512];
+#define TRACE(role, ev, it)                                                    \
+  do {                                                                         \
+    if (blockIdx.x == 0 && (it) < 512) g_bwd_trace[role][ev][it] = clock64();  \
+  } while (0)
+#else
+#define TRACE(role, ev, it) do {} while (0)
+#endif
+
 struct BwdParams {
   SchedView sv;     // units = key-tile items x n_kv_heads
   int32_t n_kv_heads, group;
@@ -61,12 +72,12 @@ struct BwdSmem {
   static constexpr int kLseOff = kDQOff + 2 * kTile * 128;   // [2 stages][128] lse*log2e
   static constexpr int kDeltaOff = kLseOff + 2 * kTile * 4;  // [2 stages][128] delta*scale
   static constexpr int kBarOff = kDeltaOff + 2 * kTile * 4;
-  // kv_full kv_empty q_full[2] q_empty[2] do_full do_empty s_full p_full dp_full ds_full dq_full
+  // k_full k_empty (+ v_full v_empty at the end) q_full[2] q_empty[2] do_full do_empty s_full p_full dp_full ds_full dq_full
   // dq_drained acc_full acc_empty
-  static constexpr int kNumBars = 16;
+  static constexpr int kNumBars = 18;
   static constexpr int kTmemSlotOff = kBarOff + kNumBars * 8;
   static constexpr int kSchedOff = kTmemSlotOff + 16;
-  static constexpr int kBytes = kSchedOff + 64;
+  static constexpr int kBytes = kSchedOff + kSchedRingBytes;
 };
 
 // Iterations of one item: for each query head of the group, for each span (query range), the
@@ -157,16 +168,25 @@ __device__ __forceinline__ void issue_dq(uint32_t tmem_d, uint32_t ds_addr, uint
 
 namespace {
 
+// all lanes of a converged warp have finished their part: one arrival for the warp
+__device__ __forceinline__ void warp_arrive(uint64_t* bar) {
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
+}
+
 template <int D>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmDO,
-                const __grid_constant__ CUtensorMap tmDQ, const __grid_constant__ BwdParams p) {
+                const __grid_constant__ CUtensorMap tmDQ, const __grid_constant__ CUtensorMap tmDK,
+                const __grid_constant__ CUtensorMap tmDV, const __grid_constant__ BwdParams p) {
   using L = BwdSmem<D>;
   extern __shared__ __align__(1024) uint8_t smem[];
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + L::kBarOff);
-  uint64_t* kv_full = bars + 0;
-  uint64_t* kv_empty = bars + 1;
+  uint64_t* k_full = bars + 0;
+  uint64_t* k_empty = bars + 1;
+  uint64_t* v_full = bars + 16;
+  uint64_t* v_empty = bars + 17;
   uint64_t* q_full = bars + 2;   // [2]
   uint64_t* q_empty = bars + 4;  // [2]
   uint64_t* do_full = bars + 6;
@@ -190,9 +210,11 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     __trap();
   }
   if (warp == 9 && lane == 0) {
-    sched_ring_init(sched, kComputeThreads + 1);  // consumers: compute threads + the MMA lane
-    mbar_init(kv_full, 1);
-    mbar_init(kv_empty, 1);
+    sched_ring_init(sched, kComputeThreads + 2);  // compute threads + the MMA lane + the TMA lane
+    mbar_init(k_full, 1);
+    mbar_init(k_empty, 1);
+    mbar_init(v_full, 1);
+    mbar_init(v_empty, 1);
     for (int i = 0; i < 2; ++i) {
       mbar_init(&q_full[i], 33);  // expect_tx arrive + 32 lanes staging LSE/delta
       mbar_init(&q_empty[i], 1);
@@ -200,19 +222,21 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     mbar_init(do_full, 1);
     mbar_init(do_empty, 1);
     mbar_init(s_full, 1);
-    mbar_init(p_full, kComputeThreads);
+    mbar_init(p_full, kComputeThreads / 32);  // one arrival per compute warp
     mbar_init(dp_full, 1);
-    mbar_init(ds_full, kComputeThreads);
+    mbar_init(ds_full, kComputeThreads / 32);  // one arrival per compute warp
     mbar_init(dq_full, 1);
-    mbar_init(dq_drained, kComputeThreads);
+    mbar_init(dq_drained, kComputeThreads / 32);  // one arrival per compute warp
     mbar_init(acc_full, 1);
-    mbar_init(acc_empty, kComputeThreads);
+    mbar_init(acc_empty, kComputeThreads / 32);  // one arrival per compute warp
     fence_barrier_init();
     prefetch_tensormap(&tmQ);
     prefetch_tensormap(&tmK);
     prefetch_tensormap(&tmV);
     prefetch_tensormap(&tmDO);
     prefetch_tensormap(&tmDQ);
+    prefetch_tensormap(&tmDK);
+    prefetch_tensormap(&tmDV);
   }
   if (warp == 8) tmem_alloc<512>(tmem_slot);
   tc_fence_before();
@@ -226,27 +250,36 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   if (warp == 9) {
     // ============================ TMA producer + LSE/delta staging ============================
     uint32_t item_n = 0, it_n = 0;  // items / iterations issued so far (ring phases)
-    UnitProducer prod{sched};
+    UnitConsumer cons{sched};  // lane 0 consumes; the other lanes read the slot after it
     while (true) {
-      int32_t w = 0;
-      if (lane == 0) w = prod.next(p.sv);
-      w = __shfl_sync(0xffffffffu, w, 0);
-      if (w < 0) break;
-      const Unit u = decode_unit(p.sv, w);
+      Unit u;
+      if (lane != 0) cons.wait_peek(&u);
+      __syncwarp();  // lane 0 releases the slot only after everybody has read it
+      int more = 0;
+      if (lane == 0) more = cons.next(&u);
+      more = __shfl_sync(0xffffffffu, more, 0);
+      if (lane != 0) ++cons.n;
+      if (!more) break;
       const Item& it = u.item;
       const int g = u.head;
       BwdWalker wk;
       wk.init(p.sv.spans, it, p.group);
       if (wk.done()) continue;
-      if (lane == 0) {
-        mbar_wait(kv_empty, (item_n & 1) ^ 1);
-        mbar_arrive_expect_tx(kv_full, 2 * L::kTileBytes);
-        for (int half = 0; half < D / 64; ++half) {
-          tma_load_3d(smem + L::kKOff + half * (kTile * 128), &tmK, kv_full, half * 64, g, it.row0);
-          tma_load_3d(smem + L::kVOff + half * (kTile * 128), &tmV, kv_full, half * 64, g, it.row0);
-        }
-      }
-      ++item_n;
+      // The first iteration's Q / LSE / delta / dO go out BEFORE this unit's K and V: their
+      // buffers free up well before the previous unit ends, whereas V is only released at that
+      // unit's last dP^T MMA and K at its last dQ MMA.  K/V then stream in under the previous
+      // unit's tail (dS, dK/dQ, the dQ drain and the dK/dV epilogue).
+      auto load_kv = [&]() {
+        mbar_wait(v_empty, (item_n & 1) ^ 1);
+        mbar_arrive_expect_tx(v_full, L::kTileBytes);
+        for (int half = 0; half < D / 64; ++half)
+          tma_load_3d(smem + L::kVOff + half * (kTile * 128), &tmV, v_full, half * 64, g, it.row0);
+        mbar_wait(k_empty, (item_n & 1) ^ 1);
+        mbar_arrive_expect_tx(k_full, L::kTileBytes);
+        for (int half = 0; half < D / 64; ++half)
+          tma_load_3d(smem + L::kKOff + half * (kTile * 128), &tmK, k_full, half * 64, g, it.row0);
+      };
+      bool kv_pending = true;
       for (; !wk.done(); wk.next(), ++it_n) {
         const int st = it_n & 1, h = g * p.group + wk.hi, qrow = wk.q_row();
         mbar_wait(&q_empty[st], ((it_n >> 1) & 1) ^ 1);
@@ -270,8 +303,19 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           mbar_arrive_expect_tx(do_full, L::kTileBytes);
           for (int half = 0; half < D / 64; ++half)
             tma_load_3d(smem + L::kDOOff + half * (kTile * 128), &tmDO, do_full, half * 64, h, qrow);
+          if (kv_pending) load_kv();
         }
+        kv_pending = false;
         __syncwarp();
+      }
+      ++item_n;
+    }
+  } else if (warp == 10) {
+    // ======================================== scheduler ========================================
+    if (lane == 0) {
+      UnitProducer prod{sched};
+      Unit u;
+      while (prod.next(p.sv, &u)) {
       }
     }
   } else if (warp == 8) {
@@ -279,15 +323,13 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (lane == 0) {
       uint32_t item_n = 0, it_n = 0;
       UnitConsumer cons{sched};
-      int32_t w;
-      while ((w = cons.next()) >= 0) {
-        const Unit u = decode_unit(p.sv, w);
+      Unit u;
+      while (cons.next(&u)) {
         const Item& it = u.item;
         BwdWalker wk;
         wk.init(p.sv.spans, it, p.group);
         if (wk.done()) continue;
-        mbar_wait(kv_full, item_n & 1);
-        mbar_wait(acc_empty, (item_n & 1) ^ 1);  // previous item's dK/dV have left TMEM
+        mbar_wait(k_full, item_n & 1);
         tc_fence_after();
         // prologue: S^T(0)
         mbar_wait(&q_full[it_n & 1], (it_n >> 1) & 1);
@@ -303,7 +345,12 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           // dV += P^T dO
           mbar_wait(do_full, it_n & 1);
           mbar_wait(p_full, it_n & 1);
+          if (first) {
+            mbar_wait(acc_empty, (item_n & 1) ^ 1);  // previous unit's dK/dV have left TMEM
+            mbar_wait(v_full, item_n & 1);
+          }
           tc_fence_after();
+          TRACE(2, 0, it_n);
           issue_dv<D>(tmem + 384, tmem, sDO, !first);
           // dP^T = V dO^T (its TMEM region held dQ of the previous iteration)
           if (!first) {
@@ -313,6 +360,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           issue_kmajor<D>(tmem + 128, sV, sDO);
           tc_commit(dp_full);
           tc_commit(do_empty);
+          TRACE(2, 1, it_n);
+          if (!has_next) tc_commit(v_empty);
           // S^T of the next iteration (P^T of this one has been consumed by dV, in issue order)
           if (has_next) {
             mbar_wait(&q_full[(it_n + 1) & 1], ((it_n + 1) >> 1) & 1);
@@ -321,19 +370,22 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_commit(s_full);
           }
           // dK += dS^T Q ; dQ = dS K
+          TRACE(2, 2, it_n);
           mbar_wait(ds_full, it_n & 1);
+          TRACE(2, 3, it_n);
           tc_fence_after();
           issue_dk<D>(tmem + 256, sDS, sQ + st * L::kTileBytes, !first);
           issue_dq<D>(tmem + 128, sDS, sK);
           tc_commit(dq_full);
           tc_commit(&q_empty[st]);
+          TRACE(2, 4, it_n);
           first = false;
           ++it_n;
           if (!has_next) break;
           wk = nxt;
         }
         tc_commit(acc_full);
-        tc_commit(kv_empty);
+        tc_commit(k_empty);
         ++item_n;
       }
     }
@@ -350,9 +402,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint8_t* dq_stage = smem + L::kDQOff + wg * (kTile * 128);
     uint32_t item_n = 0, it_n = 0;
     UnitConsumer cons{sched};
-    int32_t w;
-    while ((w = cons.next()) >= 0) {
-      const Unit u = decode_unit(p.sv, w);
+    Unit u;
+    while (cons.next(&u)) {
       const Item& it = u.item;
       const int g = u.head;
       const int b = it.local0 + r;  // key index inside its range
@@ -372,6 +423,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
       auto compute_p = [&](const BwdWalker& k, uint32_t n) {
         mbar_wait(s_full, n & 1);
+        if (r == 0) TRACE(wg, 0, n);
         tc_fence_after();
         uint32_t s[64];
         tmem_ld32(tS, &s[0]);
@@ -400,11 +452,13 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tmem_st32(tP, pk);
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(p_full);
+        warp_arrive(p_full);
+        if (r == 0) TRACE(wg, 1, n);
       };
 
       auto drain_dq = [&](uint32_t n) {  // dQ of iteration n -> smem -> TMA reduce-add
         mbar_wait(dq_full, n & 1);
+        if (r == 0) TRACE(wg, 4, n);
         tc_fence_after();
 #pragma unroll
         for (int c = 0; c < D / 64; ++c) {
@@ -413,7 +467,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           tmem_wait_ld();
           if (c == D / 64 - 1) {
             tc_fence_before();
-            mbar_arrive(dq_drained);
+            warp_arrive(dq_drained);
           }
           if (r == 0) bulk_wait_group_read<0>();  // the previous reduce has read the staging tile
           bar_sync(1 + wg, 128);
@@ -438,6 +492,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (!first) drain_dq(it_n - 1);
         // dS^T = P^T * (dP^T * scale - delta * scale)
         mbar_wait(dp_full, it_n & 1);
+        if (r == 0) TRACE(wg, 2, it_n);
         tc_fence_after();
         {
           uint32_t dp[64];
@@ -464,7 +519,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
         fence_proxy_async_smem();
         tc_fence_before();
-        mbar_arrive(ds_full);
+        warp_arrive(ds_full);
+        if (r == 0) TRACE(wg, 3, it_n);
         prev_h = g * p.group + wk.hi;
         prev_qrow = wk.q_row();
         first = false;
@@ -475,15 +531,31 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       }
       drain_dq(it_n - 1);
       // ------------------------------ epilogue: dK (WG A), dV (WG B) ------------------------------
+      if (r == 0) TRACE(wg, 5, it_n - 1);
       mbar_wait(acc_full, item_n & 1);
+      if (r == 0) TRACE(wg, 6, it_n - 1);
       tc_fence_after();
       const uint32_t tAcc = tmem + lane_addr + 256 + wg * 128;
+      if (it.local0 + kTile <= it.range_len) {
+        // Full key tile: 32 columns at a time through this warpgroup's half of the dQ staging
+        // area (two 8 KB buffers) and out with TMA stores - whole 64-byte row segments, no LSU
+        // work.  (Row-per-thread 16-byte global stores cost one half-used sector each: ~5000
+        // cycles per unit, measured.)
+        uint8_t* stg = smem + L::kDQOff + wg * (kTile * 128);
 #pragma unroll
-      for (int c = 0; c < D / 32; ++c) {
-        uint32_t v[32];
-        tmem_ld32(tAcc + c * 32, v);
-        tmem_wait_ld();
-        if (key_ok) {
+        for (int c = 0; c < D / 32; ++c) {
+          uint32_t v[32];
+          tmem_ld32(tAcc + c * 32, v);
+          tmem_wait_ld();
+          if (c == D / 32 - 1) {  // the accumulators have left TMEM
+            tc_fence_before();
+            warp_arrive(acc_empty);
+          }
+          if (r == 0) {  // the buffer's previous reader (dQ reduce or the store two chunks back)
+            if (c == 0) bulk_wait_group_read<0>(); else bulk_wait_group_read<1>();
+          }
+          bar_sync(1 + wg, 128);
+          uint8_t* row = stg + (c & 1) * 8192 + r * 64;
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
             uint4 pk;
@@ -491,12 +563,38 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             pk.y = pack_bf16(__uint_as_float(v[8 * q + 2]), __uint_as_float(v[8 * q + 3]));
             pk.z = pack_bf16(__uint_as_float(v[8 * q + 4]), __uint_as_float(v[8 * q + 5]));
             pk.w = pack_bf16(__uint_as_float(v[8 * q + 6]), __uint_as_float(v[8 * q + 7]));
-            reinterpret_cast<uint4*>(out)[c * 4 + q] = pk;
+            *reinterpret_cast<uint4*>(row + q * 16) = pk;
+          }
+          fence_proxy_async_smem();
+          bar_sync(1 + wg, 128);
+          if (r == 0) {
+            tma_store_3d(wg == 0 ? &tmDK : &tmDV, stg + (c & 1) * 8192, c * 32, g, it.row0);
+            bulk_commit_group();
           }
         }
+      } else {
+        // ragged last tile of a key range: rows past the range belong to somebody else
+#pragma unroll
+        for (int c = 0; c < D / 32; ++c) {
+          uint32_t v[32];
+          tmem_ld32(tAcc + c * 32, v);
+          tmem_wait_ld();
+          if (key_ok) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              uint4 pk;
+              pk.x = pack_bf16(__uint_as_float(v[8 * q + 0]), __uint_as_float(v[8 * q + 1]));
+              pk.y = pack_bf16(__uint_as_float(v[8 * q + 2]), __uint_as_float(v[8 * q + 3]));
+              pk.z = pack_bf16(__uint_as_float(v[8 * q + 4]), __uint_as_float(v[8 * q + 5]));
+              pk.w = pack_bf16(__uint_as_float(v[8 * q + 6]), __uint_as_float(v[8 * q + 7]));
+              reinterpret_cast<uint4*>(out)[c * 4 + q] = pk;
+            }
+          }
+        }
+        tc_fence_before();
+        warp_arrive(acc_empty);
       }
-      tc_fence_before();
-      mbar_arrive(acc_empty);
+      if (r == 0) TRACE(wg, 7, it_n - 1);
       ++item_n;
     }
     if (r == 0) bulk_wait_group<0>();  // all dQ reductions have landed before the CTA exits
@@ -507,6 +605,12 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 }
 
 }  // namespace
+
+#ifdef BS_BWD_TRACE
+extern "C" int bs_debug_bwd_trace(long long* host_out) {
+  return (int)cudaMemcpyFromSymbol(host_out, g_bwd_trace, sizeof(g_bwd_trace));
+}
+#endif
 
 extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, const void* K,
                                    const void* V, const void* dO, const float* LSE_final,
@@ -536,7 +640,7 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   if (tb.items.empty()) return BS_OK;
 
   const int D = shape->head_dim;
-  CUtensorMap tmQ, tmK, tmV, tmDO, tmDQ;
+  CUtensorMap tmQ, tmK, tmV, tmDO, tmDQ, tmDK, tmDV;
   rc = bs::make_tensor_map_3d(&tmQ, Q, 2, D, shape->n_q_heads, shape->q_rows, shape->q_row_stride,
                               64, bs::kTile, true);
   if (rc != BS_OK) return rc;
@@ -551,6 +655,13 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmDQ, dQ_acc, 4, D, shape->n_q_heads, shape->q_rows,
                               (int64_t)shape->n_q_heads * D, 32, bs::kTile, true);
+  if (rc != BS_OK) return rc;
+
+  rc = bs::make_tensor_map_3d(&tmDK, dK, 2, D, shape->n_kv_heads, shape->kv_rows,
+                              shape->kv_row_stride, 32, bs::kTile, false);
+  if (rc != BS_OK) return rc;
+  rc = bs::make_tensor_map_3d(&tmDV, dV, 2, D, shape->n_kv_heads, shape->kv_rows,
+                              shape->kv_row_stride, 32, bs::kTile, false);
   if (rc != BS_OK) return rc;
 
   BwdParams p;
@@ -570,11 +681,11 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   if (D == 128) {
     BS_CUDA(cudaFuncSetAttribute(attn_bwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  BwdSmem<128>::kBytes));
-    attn_bwd_kernel<128><<<grid, kBwdThreads, BwdSmem<128>::kBytes, st>>>(tmQ, tmK, tmV, tmDO, tmDQ, p);
+    attn_bwd_kernel<128><<<grid, kBwdThreads, BwdSmem<128>::kBytes, st>>>(tmQ, tmK, tmV, tmDO, tmDQ, tmDK, tmDV, p);
   } else {
     BS_CUDA(cudaFuncSetAttribute(attn_bwd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  BwdSmem<64>::kBytes));
-    attn_bwd_kernel<64><<<grid, kBwdThreads, BwdSmem<64>::kBytes, st>>>(tmQ, tmK, tmV, tmDO, tmDQ, p);
+    attn_bwd_kernel<64><<<grid, kBwdThreads, BwdSmem<64>::kBytes, st>>>(tmQ, tmK, tmV, tmDO, tmDQ, tmDK, tmDV, p);
   }
   BS_CUDA(cudaGetLastError());
   bs::count_launch();

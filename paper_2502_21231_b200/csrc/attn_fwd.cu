@@ -29,7 +29,7 @@ using namespace bs;
 using namespace bs::ptx;
 
 constexpr int kFwdThreads = 640;      // 4 softmax warpgroups + 1 auxiliary warpgroup (MMA, TMA)
-constexpr int kMmaWarp0 = 16, kTmaWarp = 17;  // warps 16 / 18 issue the MMAs of Q tile 0 / 1
+constexpr int kMmaWarp0 = 16, kTmaWarp = 17, kSchedWarp = 19;  // warps 16 / 18 issue the MMAs of Q tile 0 / 1
 constexpr int kRegsSoftmax = 104;     // setmaxnreg: 512 * 104 + 128 * 96 = 65536 (compiled at 96)
 constexpr int kStages = 4;              // K/V ring depth (K and V blocks alternate in the ring)
 constexpr float kRescaleThreshold = 8.f;  // log2 units
@@ -58,12 +58,15 @@ __device__ __forceinline__ float2 ex2_fma2(float2 x) {
 #ifdef BS_FWD_TRACE
 // debug build only: per-event clock64() stamps of CTA 0 (role, event) x iteration
 __device__ long long g_fwd_trace[4][8][256];
+__device__ long long g_fwd_utrace[5][8][64];  // per unit: softmax thread 0 of tile t
+#define UTRACE(t, ev, n) do { if (blockIdx.x == 0 && (n) < 64) g_fwd_utrace[t][ev][n] = clock64(); } while (0)
 #define TRACE(role, ev, it)                                                    \
   do {                                                                         \
     if (blockIdx.x == 0 && (it) < 256) g_fwd_trace[role][ev][it] = clock64();  \
   } while (0)
 #else
 #define TRACE(role, ev, it) do {} while (0)
+#define UTRACE(t, ev, n) do {} while (0)
 #endif
 
 struct FwdParams {
@@ -85,8 +88,8 @@ struct FwdSmem {
   // barriers: q_full[2], q_empty[2], kv_full[S], kv_empty[S], s_full[2], p_full[2][2], o_full[2]
   static constexpr int kNumBars = 4 + 2 * kStages + 8;
   static constexpr int kTmemSlotOff = kBarOff + kNumBars * 8;
-  static constexpr int kSchedOff = kTmemSlotOff + 8;  // SchedRing of the dynamic scheduler
-  static constexpr int kXchOff = kSchedOff + 64;      // row max [2 tiles][2][2][128], row sum [2][2][128]
+  static constexpr int kSchedOff = kTmemSlotOff + 16;  // SchedRing of the dynamic scheduler
+  static constexpr int kXchOff = kSchedOff + kSchedRingBytes;     // row max [2 tiles][2][2][128], row sum [2][2][128]
   static constexpr int kLockOff = kXchOff + 6144;     // turn lock of the two MMA issuers
   static constexpr int kBytes = kLockOff + 16;
   static constexpr int kAlloc = kBytes + 1024;  // slack to align the base to 1024 B
@@ -213,7 +216,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
   if (warp == kTmaWarp && lane == 0) {
     *reinterpret_cast<uint32_t*>(smem + L::kLockOff) = 0;
-    sched_ring_init(sched, 4 * kTile + 2);  // consumers: 512 softmax threads + 2 MMA lanes
+    sched_ring_init(sched, 4 * kTile + 3);  // 512 softmax threads + 2 MMA lanes + the TMA lane  // consumers: 512 softmax threads + 2 MMA lanes
     for (int t = 0; t < 2; ++t) {
       mbar_init(&q_full[t], 1);
       mbar_init(&q_empty[t], 1);
@@ -243,31 +246,39 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       // ===================================== TMA producer =====================================
       uint32_t q_ph[2] = {0, 0};
       Ring ring;
-      UnitProducer prod{sched};
-      int32_t w;
-      while ((w = prod.next(p.sv)) >= 0) {
-        const Unit u = decode_unit(p.sv, w);
+      UnitConsumer cons{sched};
+      Unit u;
+      int un = -1;
+      while (cons.next(&u)) {
+        ++un;
+        UTRACE(4, 0, un);
         const Item& it = u.item;
         const int h = u.head, g = h / p.group;
         Walker wk;
         wk.init(p.sv.spans, it);
         if (wk.done()) continue;
-        // the first K/V block goes out before the Q tiles: the ring usually has room while the
-        // Q buffers are still held by the previous unit's last S MMAs
+        // Order of a unit's loads: K of the first block (its ring stage is released early, at
+        // the S MMAs four stages back), then the two Q tiles (a tile's buffer is released at its
+        // last S MMA of the previous unit), then V of the first block and the rest.  V stages are
+        // only released at PV MMAs, i.e. late in the previous unit: nothing S(0) needs may queue
+        // behind them.
+        auto load_kv = [&](int kv, int krow) {
+          mbar_wait(&kv_empty[ring.stage], ring.phase ^ 1);
+          mbar_arrive_expect_tx(&kv_full[ring.stage], L::kTileBytes);
+          for (int half = 0; half < D / 64; ++half)
+            tma_load_3d(smem + L::kKVOff + ring.stage * L::kTileBytes + half * (kTile * 128),
+                        kv == 0 ? &tmK : &tmV, &kv_full[ring.stage], half * 64, g, krow);
+          ring.advance();
+        };
         for (bool first = true; !wk.done(); wk.next(), first = false) {
           const int krow = wk.sp.begin + wk.j * kTile;
-          for (int kv = 0; kv < 2; ++kv) {
-            mbar_wait(&kv_empty[ring.stage], ring.phase ^ 1);
-            mbar_arrive_expect_tx(&kv_full[ring.stage], L::kTileBytes);
-            for (int half = 0; half < D / 64; ++half)
-              tma_load_3d(smem + L::kKVOff + ring.stage * L::kTileBytes + half * (kTile * 128),
-                          kv == 0 ? &tmK : &tmV, &kv_full[ring.stage], half * 64, g, krow);
-            ring.advance();
-          }
+          load_kv(0, krow);
           if (first) {
+            UTRACE(4, 1, un);
             for (int t = 0; t < 2; ++t) {
               if (wk.total(t) == 0) continue;
               mbar_wait(&q_empty[t], q_ph[t] ^ 1);
+              UTRACE(4, 2 + t, un);
               q_ph[t] ^= 1;
               mbar_arrive_expect_tx(&q_full[t], L::kTileBytes);
               for (int half = 0; half < D / 64; ++half)
@@ -275,7 +286,16 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             &q_full[t], half * 64, h, it.row0 + t * kTile);
             }
           }
+          load_kv(1, krow);
+          if (first) UTRACE(4, 4, un);
         }
+        UTRACE(4, 5, un);
+      }
+    } else if (warp == kSchedWarp && lane == 0) {
+      // ====================================== scheduler ======================================
+      UnitProducer prod{sched};
+      Unit u;
+      while (prod.next(p.sv, &u)) {
       }
     } else if ((warp == kMmaWarp0 || warp == kMmaWarp0 + 2) && lane == 0) {
       // ============================ MMA issuer of Q tile t = 0 / 1 ============================
@@ -288,13 +308,16 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       int tr_it = 0;
       Ring ring;
       UnitConsumer cons{sched};
-      int32_t w;
-      while ((w = cons.next()) >= 0) {
-        const Unit u = decode_unit(p.sv, w);
+      Unit u;
+      int un = -1;
+      while (cons.next(&u)) {
+        ++un;
+        UTRACE(2 + t, 0, un);
         Walker cur;
         cur.init(p.sv.spans, u.item);
         if (cur.done()) continue;
         const int tot = cur.total(t);
+        UTRACE(2 + t, 1, un);
         int n_s = 0, n_pv = 0;
         auto wait_q = [&]() {  // never called with the turn lock held
           if (n_s == 0) {
@@ -319,10 +342,13 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // prologue: S_t(0).  Every ring stage is waited for and released by both issuers, also
         // for blocks their tile takes no part in.
         mbar_wait(&kv_full[ring.stage], ring.phase);
+        UTRACE(2 + t, 2, un);
         tc_fence_after();
         if (cur.active(t)) {
           wait_q();
+          UTRACE(2 + t, 3, un);
           issue_s(ring.stage);
+          UTRACE(2 + t, 4, un);
         }
         release(ring.stage);
         ring.advance();
@@ -392,9 +418,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint32_t s_ph = 0, o_ph = 0;
     int tr_it = 0;
     UnitConsumer cons{sched};
-    int32_t w;
-    while ((w = cons.next()) >= 0) {
-      const Unit u = decode_unit(p.sv, w);
+    Unit u;
+    int un = -1;
+    while (cons.next(&u)) {
+      ++un;
+      if (r == 0 && hf == 0) UTRACE(t, 0, un);
       const Item& it = u.item;
       const int h = u.head;
       Walker wk;
@@ -419,6 +447,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_wait(&s_full[t], s_ph);
         s_ph ^= 1;
         if (r == 0) TRACE(t, 0, tr_it);
+        if (r == 0 && hf == 0 && cnt == 0) UTRACE(t, 1, un);
         tc_fence_after();
         // Two passes over this thread's 64 columns in chunks of 16, double-buffered in A / B so
         // that the TMEM load of the next chunk runs under the arithmetic of the current one.
@@ -526,12 +555,14 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       }
       // ------------------------------------ epilogue ------------------------------------
       // rows that saw no key: the emulated exp2 leaves ~2^-125 per masked score in l
+      if (r == 0 && hf == 0) UTRACE(t, 2, un);
       const float l_half = m_used == -CUDART_INF_F ? 0.f : l2.x + l2.y;
       xch_l[hf * 128] = l_half;
       bar_sync(1 + t, 2 * kTile);
       const float l = l_half + xch_l[(hf ^ 1) * 128];
       mbar_wait(&o_full[t], o_ph);
       o_ph ^= 1;
+      if (r == 0 && hf == 0) UTRACE(t, 3, un);
       tc_fence_after();
       const float inv_l = l > 0.f ? 1.f / l : 0.f;
 #pragma unroll
@@ -554,6 +585,10 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       if (valid && hf == 0)
         p.LSE[(int64_t)h * p.lse_head_stride + grow] =
             l > 0.f ? m_used * 0.69314718055994531f + __logf(l) : -CUDART_INF_F;
+      if (r == 0 && hf == 0) UTRACE(t, 4, un);
+#ifdef BS_FWD_TRACE
+      if (r == 0 && hf == 0 && blockIdx.x == 0 && un < 64) g_fwd_utrace[t][5][un] = tot;
+#endif
       tc_fence_before();
     }
   }
@@ -616,6 +651,9 @@ int sm_count() {
 #ifdef BS_FWD_TRACE
 extern "C" int bs_debug_fwd_trace(long long* host_out) {
   return (int)cudaMemcpyFromSymbol(host_out, g_fwd_trace, sizeof(g_fwd_trace));
+}
+extern "C" int bs_debug_fwd_utrace(long long* host_out) {
+  return (int)cudaMemcpyFromSymbol(host_out, g_fwd_utrace, sizeof(g_fwd_utrace));
 }
 #endif
 

@@ -1,6 +1,8 @@
-// sched.cuh — device side of the persistent tile scheduler: one warp of the CTA
-// pulls unit indices from the global atomic cursor and hands them to the other warps through a
-// two-slot shared-memory ring, so every role of a warp-specialised kernel walks the same units.
+// sched.cuh — device side of the persistent tile scheduler: a scheduler warp of
+// the CTA pulls unit indices from the global atomic cursor, decodes them and hands them to the
+// other warps through a four-slot shared-memory ring, so that every role of a warp-specialised
+// kernel walks the same units and the cursor / table latency (several microseconds of dependent
+// L2 round trips) stays off the critical path of short units.
 // The cursor order is the host's longest-first / locality order (worklist.h).
 #pragma once
 #include "ptx.cuh"
@@ -21,13 +23,12 @@ struct Unit {
   int32_t head;
 };
 
-// unit index -> (item, head): binary search of the group, then head-major inside the group.
-__device__ __forceinline__ Unit decode_unit(const SchedView& sv, int32_t w) {
-  int lo = 0, hi = sv.n_groups - 1;
-  while (lo < hi) {
-    const int mid = (lo + hi + 1) >> 1;
-    if (sv.groups[mid].unit_begin <= w) lo = mid; else hi = mid - 1;
-  }
+// unit index -> (item, head): find the group (a CTA's unit indices only grow, so the search
+// walks forward from the group of its previous unit: *hint), then head-major inside the group.
+__device__ __forceinline__ Unit decode_unit(const SchedView& sv, int32_t w, int32_t* hint) {
+  int lo = *hint;
+  while (lo + 1 < sv.n_groups && sv.groups[lo + 1].unit_begin <= w) ++lo;
+  *hint = lo;
   const Group g = sv.groups[lo];
   const int local = w - g.unit_begin;
   Unit u;
@@ -36,14 +37,22 @@ __device__ __forceinline__ Unit decode_unit(const SchedView& sv, int32_t w) {
   return u;
 }
 
-constexpr int kSchedSlots = 2;
+#ifndef BS_SCHED_SLOTS
+#define BS_SCHED_SLOTS 4
+#endif
+constexpr int kSchedSlots = BS_SCHED_SLOTS;
 
-struct SchedRing {  // lives in shared memory
-  uint64_t full[kSchedSlots], empty[kSchedSlots];
+struct SchedRing {  // lives in shared memory (16-byte aligned)
+  Item item[kSchedSlots];  // decoded by the producer: consumers never touch the global tables
+  int32_t head[kSchedSlots];
   int32_t unit[kSchedSlots];
+  uint64_t full[kSchedSlots], empty[kSchedSlots];
 };
+constexpr int kSchedRingBytes = 256;
+static_assert(sizeof(SchedRing) <= kSchedRingBytes, "SchedRing size");
 
-// n_consumers = threads that call UnitConsumer::next()
+// n_consumers = arrivals per slot on the empty barrier (threads calling next(), warps calling
+// next_warp())
 __device__ __forceinline__ void sched_ring_init(SchedRing* r, uint32_t n_consumers) {
   for (int i = 0; i < kSchedSlots; ++i) {
     ptx::mbar_init(&r->full[i], 1);
@@ -51,19 +60,35 @@ __device__ __forceinline__ void sched_ring_init(SchedRing* r, uint32_t n_consume
   }
 }
 
-struct UnitProducer {  // one thread
+struct UnitProducer {  // one thread (the scheduler warp's lane 0)
   SchedRing* r;
   uint32_t n = 0;
-  // Returns the next unit index of this CTA, or -1 when the cursor ran out (also published).
-  __device__ __forceinline__ int32_t next(const SchedView& sv) {
+  int32_t hint = 0, last = 0;
+  // Pulls the next unit of this CTA from the global cursor, decodes it and publishes it.
+  // Returns false when the cursor ran out (also published, as unit -1).
+  // Look-ahead: up to kSchedSlots - 1 units beyond the one the slowest consumer works on while
+  // plenty of units are left; once the cursor is within 4 rounds of the end a unit is only
+  // claimed when every consumer has taken the previous one, so that the short tail units go to
+  // whichever CTA is free first (greedy longest-first).
+  __device__ __forceinline__ bool next(const SchedView& sv, Unit* u) {
+    if (n > 0 && last >= sv.n_units - 4 * (int32_t)gridDim.x) {
+      const uint32_t pslot = (n - 1) % kSchedSlots, pph = ((n - 1) / kSchedSlots) & 1;
+      ptx::mbar_wait(&r->empty[pslot], pph);
+    }
     int32_t w = atomicAdd(sv.counter, 1);
+    last = w;
     if (w >= sv.n_units) w = -1;
+    if (w >= 0) *u = decode_unit(sv, w, &hint);
     const uint32_t slot = n % kSchedSlots, ph = (n / kSchedSlots) & 1;
     ptx::mbar_wait(&r->empty[slot], ph ^ 1);
+    if (w >= 0) {
+      r->item[slot] = u->item;
+      r->head[slot] = u->head;
+    }
     r->unit[slot] = w;
     ptx::mbar_arrive(&r->full[slot]);
     ++n;
-    return w;
+    return w >= 0;
   }
 };
 
@@ -77,36 +102,26 @@ __device__ __forceinline__ T warp_uniform(T v) {
 struct UnitConsumer {  // every consuming thread
   SchedRing* r;
   uint32_t n = 0;
-  __device__ __forceinline__ int32_t next() {
+  __device__ __forceinline__ bool next(Unit* u) {
     const uint32_t slot = n % kSchedSlots, ph = (n / kSchedSlots) & 1;
     ptx::mbar_wait(&r->full[slot], ph);
     const int32_t w = r->unit[slot];
+    if (w >= 0) {
+      u->item = r->item[slot];
+      u->head = r->head[slot];
+    }
     ptx::mbar_arrive(&r->empty[slot]);
     ++n;
-    return w;
+    return w >= 0;
   }
-  // Whole converged warp consumes as ONE consumer (one arrival on the empty barrier).
-  __device__ __forceinline__ int32_t next_warp() {
+  // Wait for slot n and read it without consuming it (lanes 1-31 of a warp whose lane 0
+  // consumes for the warp afterwards).
+  __device__ __forceinline__ void wait_peek(Unit* u) const {
     const uint32_t slot = n % kSchedSlots, ph = (n / kSchedSlots) & 1;
-    ptx::mbar_wait_warp(&r->full[slot], ph);
-    const int32_t w = warp_uniform(r->unit[slot]);
-    __syncwarp();
-    if (ptx::elect_one()) ptx::mbar_arrive(&r->empty[slot]);
-    ++n;
-    return w;
+    ptx::mbar_wait(&r->full[slot], ph);
+    u->item = r->item[slot];
+    u->head = r->head[slot];
   }
 };
-
-// decode_unit for a converged warp: every lane loads the same words; the fields come back uniform.
-__device__ __forceinline__ Unit decode_unit_warp(const SchedView& sv, int32_t w) {
-  Unit u = decode_unit(sv, w);
-  u.head = warp_uniform(u.head);
-  u.item.row0 = warp_uniform(u.item.row0);
-  u.item.local0 = warp_uniform(u.item.local0);
-  u.item.range_len = warp_uniform(u.item.range_len);
-  u.item.span_begin = warp_uniform(u.item.span_begin);
-  u.item.n_spans = warp_uniform(u.item.n_spans);
-  return u;
-}
 
 }  // namespace bs
