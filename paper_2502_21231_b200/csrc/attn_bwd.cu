@@ -320,7 +320,10 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     }
   } else if (warp == 8) {
     // ======================================= MMA issuer =======================================
-    if (lane == 0) {
+    // (elect_one, not lane == 0: the compiler then knows a single thread runs the region and
+    // keeps the MMA descriptors in uniform registers - back-to-back UTCHMMA instead of a
+    // broadcast loop of ~16 instructions per MMA, which made the issue itself the bottleneck)
+    if (elect_one()) {
       uint32_t item_n = 0, it_n = 0;
       UnitConsumer cons{sched};
       Unit u;

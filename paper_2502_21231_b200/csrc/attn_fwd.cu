@@ -297,7 +297,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       Unit u;
       while (prod.next(p.sv, &u)) {
       }
-    } else if ((warp == kMmaWarp0 || warp == kMmaWarp0 + 2) && lane == 0) {
+    } else if ((warp == kMmaWarp0 || warp == kMmaWarp0 + 2) && elect_one()) {
       // ============================ MMA issuer of Q tile t = 0 / 1 ============================
       // Each tile has its own issuing warp (one lane).
       const int t = (warp - kMmaWarp0) >> 1;
@@ -366,8 +366,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           }
           tc_fence_after();
           if (cur.active(t)) {
-            mbar_wait(&p_full[2 * t], p_ph);      // the two column halves of P
-            mbar_wait(&p_full[2 * t + 1], p_ph);
+            mbar_wait_spin(&p_full[2 * t], p_ph);      // the two column halves of P
+            mbar_wait_spin(&p_full[2 * t + 1], p_ph);
             p_ph ^= 1;
             if (lane == 0) TRACE(2 + t, 0, tr_it);
             tc_fence_after();
@@ -518,6 +518,13 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const float2 nm2 = make_float2(neg_m, neg_m);
         auto exp16 = [&](const float* v, int k) {
           uint32_t pk[8];
+#if defined(BS_FWD_EXPERIMENT) && BS_FWD_EXPERIMENT == 1
+#pragma unroll
+          for (int i = 0; i < 8; ++i) pk[i] = 0x3c003c00u;  // experiment: no arithmetic at all
+          l2.x += v[0];
+          tmem_st8(tS + 16 * k, pk);
+          return;
+#endif
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
             const float2 x = fma2(make_float2(v[2 * i], v[2 * i + 1]), sc2, nm2);
@@ -527,7 +534,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           }
           tmem_st8(tS + 16 * k, pk);
         };
-#ifndef BS_FWD_NORELOAD
+#if !defined(BS_FWD_NORELOAD) && !(defined(BS_FWD_EXPERIMENT) && BS_FWD_EXPERIMENT == 2)
 #define RELOAD(addr, dst) tmem_ld16(addr, reinterpret_cast<uint32_t*>(dst))
 #else
 #define RELOAD(addr, dst) do {} while (0)  /* experiment only: wrong results */

@@ -138,6 +138,29 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   }
 }
 
+// Latency-critical wait: polls with test_wait (no hardware suspend between polls).  For the few
+// hand-offs on the softmax <-> MMA chain, where the wake-up delay of try_wait is on the critical
+// path; bounded like mbar_wait.
+__device__ __forceinline__ void mbar_wait_spin(uint64_t* bar, uint32_t parity) {
+  uint32_t ok = 0, spins = 0;
+  const uint32_t a = smem_u32(bar);
+  while (true) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}\n"
+        : "=r"(ok)
+        : "r"(a), "r"(parity)
+        : "memory");
+    if (ok) break;
+    if (++spins > (1u << 28)) {
+      printf("bs: mbarrier spin wait timed out (block %d thread %d bar %u parity %u)\n", blockIdx.x,
+             threadIdx.x, a, parity);
+      __trap();
+    }
+  }
+}
+
 // Converged-warp wait: one lane polls (keeps the shared-memory pipe quiet for the tensor core's
 // operand reads), the others park at the warp barrier.
 __device__ __forceinline__ void mbar_wait_warp(uint64_t* bar, uint32_t parity) {
