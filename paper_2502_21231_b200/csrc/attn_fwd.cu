@@ -17,6 +17,8 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
+#include <type_traits>
+
 #include "common.h"
 #include "launch_utils.h"
 #include "ptx.cuh"
@@ -458,11 +460,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // last visible column of this row relative to this thread's first column (>= 63: all)
         const int lim = edge ? min(at0 + r + wk.sp.off, wk.sp.len - 1) - b0 - hf * 64 : 64;
         float A[16], B[16];
-        auto mask16 = [&](float* v, int lim_k) {
-#pragma unroll
-          for (int c = 0; c < 16; ++c)
-            if (c > lim_k) v[c] = -CUDART_INF_F;
-        };
         float mx0 = -CUDART_INF_F, mx1 = -CUDART_INF_F;
         auto max16 = [&](const float* v) {
 #pragma unroll
@@ -471,22 +468,22 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             mx1 = fmax3(mx1, v[c + 2], v[c + 3]);
           }
         };
+        // Pass 1 takes the maximum over ALL 64 columns, masked or not: the running maximum is
+        // only a scaling reference (any finite value >= the visible maximum is exact in exact
+        // arithmetic), masked scores are ordinary finite q.k products of the same distribution,
+        // and the masking itself happens in pass 2, where a masked P must be 0.
         tmem_ld16(tS, reinterpret_cast<uint32_t*>(A));
         tmem_wait_ld();
         tmem_ld16(tS + 16, reinterpret_cast<uint32_t*>(B));
-        if (lim < 15) mask16(A, lim);
         max16(A);
         tmem_wait_ld();
         tmem_ld16(tS + 32, reinterpret_cast<uint32_t*>(A));
-        if (lim < 31) mask16(B, lim - 16);
         max16(B);
         tmem_wait_ld();
         tmem_ld16(tS + 48, reinterpret_cast<uint32_t*>(B));
-        if (lim < 47) mask16(A, lim - 32);
         max16(A);
         tmem_wait_ld();
-        if (lim < 63) mask16(B, lim - 48);
-        max16(B);
+        max16(B);  // chunk 3 stays in B for pass 2
         if (r == 0) TRACE(t, 1, tr_it);
         const float mx_half = fmaxf(mx0, mx1);
         // exchange the half-row maxima (slots alternate with the block parity; one barrier/block)
@@ -516,23 +513,27 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (r == 0) TRACE(t, 2, tr_it);
         const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
         const float2 nm2 = make_float2(neg_m, neg_m);
-        auto exp16 = [&](const float* v, int k) {
+        // P of one 16-column chunk.  Masked columns (c > lim_k) are zeroed AFTER the exponential,
+        // so that a masked P is exactly 0 whichever exp2 path produced it.
+        auto exp16_body = [&](const float* v, int k, int lim_k, auto masked) {
           uint32_t pk[8];
-#if defined(BS_FWD_EXPERIMENT) && BS_FWD_EXPERIMENT == 1
-#pragma unroll
-          for (int i = 0; i < 8; ++i) pk[i] = 0x3c003c00u;  // experiment: no arithmetic at all
-          l2.x += v[0];
-          tmem_st8(tS + 16 * k, pk);
-          return;
-#endif
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
             const float2 x = fma2(make_float2(v[2 * i], v[2 * i + 1]), sc2, nm2);
-            const float2 e = (i & 3) < kEmuOf4 ? ex2_fma2(x) : make_float2(ex2(x.x), ex2(x.y));
+            float2 e = (i & 3) < kEmuOf4 ? ex2_fma2(x) : make_float2(ex2(x.x), ex2(x.y));
+            if (decltype(masked)::value) {
+              if (2 * i > lim_k) e.x = 0.f;
+              if (2 * i + 1 > lim_k) e.y = 0.f;
+            }
             l2 = add2(l2, e);
             pk[i] = pack_bf16(e.x, e.y);
           }
           tmem_st8(tS + 16 * k, pk);
+        };
+        // (`edge` is the same for the whole warp: tcgen05.st must not sit in divergent code)
+        auto exp16 = [&](const float* v, int k, int lim_k) {
+          if (!edge) exp16_body(v, k, lim_k, std::false_type{});
+          else exp16_body(v, k, lim_k, std::true_type{});
         };
 #if !defined(BS_FWD_NORELOAD) && !(defined(BS_FWD_EXPERIMENT) && BS_FWD_EXPERIMENT == 2)
 #define RELOAD(addr, dst) tmem_ld16(addr, reinterpret_cast<uint32_t*>(dst))
@@ -540,18 +541,15 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #define RELOAD(addr, dst) do {} while (0)  /* experiment only: wrong results */
 #endif
         RELOAD(tS, A);
-        exp16(B, 3);
+        exp16(B, 3, lim - 48);
         tmem_wait_ld();
         RELOAD(tS + 16, B);
-        if (lim < 15) mask16(A, lim);
-        exp16(A, 0);
+        exp16(A, 0, lim);
         tmem_wait_ld();
         RELOAD(tS + 32, A);
-        if (lim < 31) mask16(B, lim - 16);
-        exp16(B, 1);
+        exp16(B, 1, lim - 16);
         tmem_wait_ld();
-        if (lim < 47) mask16(A, lim - 32);
-        exp16(A, 2);
+        exp16(A, 2, lim - 32);
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
