@@ -468,22 +468,31 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             mx1 = fmax3(mx1, v[c + 2], v[c + 3]);
           }
         };
-        // Pass 1 takes the maximum over ALL 64 columns, masked or not: the running maximum is
-        // only a scaling reference (any finite value >= the visible maximum is exact in exact
-        // arithmetic), masked scores are ordinary finite q.k products of the same distribution,
-        // and the masking itself happens in pass 2, where a masked P must be 0.
+        // Pass 1: maximum over the visible columns.  It has to be exact: with an inflated
+        // maximum the largest P of a row is no longer exactly 1, its bf16 rounding no longer
+        // cancels against the fp32 row sum, and rows with few visible keys (the first rows of a
+        // document) lose up to 2^-9 relative in O.  Chunks without a visible column are skipped,
+        // only the row's boundary chunk pays for selects.
+        auto max16m = [&](const float* v, int lim_k) {
+          if (!edge || lim_k >= 15) {
+            max16(v);
+          } else if (lim_k >= 0) {
+#pragma unroll
+            for (int c = 0; c < 16; ++c) mx0 = fmaxf(mx0, c <= lim_k ? v[c] : -CUDART_INF_F);
+          }
+        };
         tmem_ld16(tS, reinterpret_cast<uint32_t*>(A));
         tmem_wait_ld();
         tmem_ld16(tS + 16, reinterpret_cast<uint32_t*>(B));
-        max16(A);
+        max16m(A, lim);
         tmem_wait_ld();
         tmem_ld16(tS + 32, reinterpret_cast<uint32_t*>(A));
-        max16(B);
+        max16m(B, lim - 16);
         tmem_wait_ld();
         tmem_ld16(tS + 48, reinterpret_cast<uint32_t*>(B));
-        max16(A);
+        max16m(A, lim - 32);
         tmem_wait_ld();
-        max16(B);  // chunk 3 stays in B for pass 2
+        max16m(B, lim - 48);  // chunk 3 stays in B for pass 2
         if (r == 0) TRACE(t, 1, tr_it);
         const float mx_half = fmaxf(mx0, mx1);
         // exchange the half-row maxima (slots alternate with the block parity; one barrier/block)
@@ -513,10 +522,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (r == 0) TRACE(t, 2, tr_it);
         const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
         const float2 nm2 = make_float2(neg_m, neg_m);
-        // P of one 16-column chunk.  Masked columns (c > lim_k) are zeroed AFTER the exponential,
-        // so that a masked P is exactly 0 whichever exp2 path produced it.
-        auto exp16_body = [&](const float* v, int k, int lim_k, auto masked) {
-          uint32_t pk[8];
+        // P of one 16-column chunk: all columns visible (lim_k >= 15), none (lim_k < 0: zeros, no
+        // exponentials at all) or the one boundary chunk of the row, where masked columns are
+        // zeroed after the exponential.  The branches hold arithmetic only and may diverge
+        // between the rows of a warp; the tcgen05.st after them is converged again.
+        auto exp16_body = [&](const float* v, int lim_k, uint32_t* pk, auto masked) {
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
             const float2 x = fma2(make_float2(v[2 * i], v[2 * i + 1]), sc2, nm2);
@@ -528,12 +538,19 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             l2 = add2(l2, e);
             pk[i] = pack_bf16(e.x, e.y);
           }
-          tmem_st8(tS + 16 * k, pk);
         };
-        // (`edge` is the same for the whole warp: tcgen05.st must not sit in divergent code)
         auto exp16 = [&](const float* v, int k, int lim_k) {
-          if (!edge) exp16_body(v, k, lim_k, std::false_type{});
-          else exp16_body(v, k, lim_k, std::true_type{});
+          uint32_t pk[8];
+          if (!edge || lim_k >= 15) {  // (interior blocks: warp-uniform, no divergence at all)
+            exp16_body(v, lim_k, pk, std::false_type{});
+          } else if (lim_k < 0) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) pk[i] = 0u;
+          } else {
+            exp16_body(v, lim_k, pk, std::true_type{});
+          }
+          if (edge) __syncwarp();
+          tmem_st8(tS + 16 * k, pk);
         };
 #if !defined(BS_FWD_NORELOAD) && !(defined(BS_FWD_EXPERIMENT) && BS_FWD_EXPERIMENT == 2)
 #define RELOAD(addr, dst) tmem_ld16(addr, reinterpret_cast<uint32_t*>(dst))
