@@ -459,7 +459,12 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (r == 0) TRACE(wg, 1, n);
       };
 
-      auto drain_dq = [&](uint32_t n) {  // dQ of iteration n -> smem -> TMA reduce-add
+      // dQ of iteration n -> smem -> TMA reduce-add.  In the loop both 32-column chunks go through
+      // this warpgroup's dQ staging tile one after the other (the compute warps have slack there).
+      // After the unit's last iteration (`last`) the dS^T box of this warpgroup is free as well and
+      // takes chunk 0, so the two reduces - and the dK/dV epilogue behind them - do not queue up.
+      uint8_t* ds_box = smem + L::kDSOff + wg * (kTile * 128);
+      auto drain_dq = [&](uint32_t n, bool last) {
         mbar_wait(dq_full, n & 1);
         if (r == 0) TRACE(wg, 4, n);
         tc_fence_after();
@@ -472,16 +477,19 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_fence_before();
             warp_arrive(dq_drained);
           }
-          if (r == 0) bulk_wait_group_read<0>();  // the previous reduce has read the staging tile
+          uint8_t* stage = (last && c == 0) ? ds_box : dq_stage;
+          if (r == 0) {  // the previous reader of this staging tile is done
+            if (last) bulk_wait_group_read<1>(); else bulk_wait_group_read<0>();
+          }
           bar_sync(1 + wg, 128);
 #pragma unroll
           for (int j = 0; j < 8; ++j)
-            *reinterpret_cast<uint4*>(dq_stage + r * 128 + ((j ^ (r & 7)) * 16)) =
+            *reinterpret_cast<uint4*>(stage + r * 128 + ((j ^ (r & 7)) * 16)) =
                 make_uint4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
           fence_proxy_async_smem();
           bar_sync(1 + wg, 128);
           if (r == 0) {
-            tma_reduce_add_3d(&tmDQ, dq_stage, wg * (D / 2) + c * 32, prev_h, prev_qrow);
+            tma_reduce_add_3d(&tmDQ, stage, wg * (D / 2) + c * 32, prev_h, prev_qrow);
             bulk_commit_group();
           }
         }
@@ -492,7 +500,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         BwdWalker nxt = wk;
         nxt.next();
         const bool has_next = !nxt.done();
-        if (!first) drain_dq(it_n - 1);
+        if (!first) drain_dq(it_n - 1, false);
         // dS^T = P^T * (dP^T * scale - delta * scale)
         mbar_wait(dp_full, it_n & 1);
         if (r == 0) TRACE(wg, 2, it_n);
@@ -502,6 +510,10 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           tmem_ld32(tDP, &dp[0]);
           tmem_ld32(tDP + 32, &dp[32]);
           tmem_wait_ld();
+          if (first) {  // the previous unit's last dQ reduce / epilogue stores read this dS^T box
+            if (r == 0) bulk_wait_group_read<0>();
+            bar_sync(1 + wg, 128);
+          }
           const float* dl = delta_s + (it_n & 1) * kTile + wg * 64;
 #pragma unroll
           for (int j = 0; j < 8; ++j) {  // 8 queries = one 16-byte chunk of the dS^T row
@@ -532,7 +544,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         compute_p(nxt, it_n);
         wk = nxt;
       }
-      drain_dq(it_n - 1);
+      drain_dq(it_n - 1, true);
       // ------------------------------ epilogue: dK (WG A), dV (WG B) ------------------------------
       if (r == 0) TRACE(wg, 5, it_n - 1);
       mbar_wait(acc_full, item_n & 1);
@@ -544,21 +556,27 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // area (two 8 KB buffers) and out with TMA stores - whole 64-byte row segments, no LSU
         // work.  (Row-per-thread 16-byte global stores cost one half-used sector each: ~5000
         // cycles per unit, measured.)
-        uint8_t* stg = smem + L::kDQOff + wg * (kTile * 128);
+        // staging: D = 128: chunks 0,1 in the dS^T box (after the last drain's chunk-0 reduce),
+        // chunks 2,3 in the dQ staging tile (after its chunk-1 reduce); D = 64: the dQ staging tile
+        constexpr int kChunks = D / 32;
 #pragma unroll
-        for (int c = 0; c < D / 32; ++c) {
+        for (int c = 0; c < kChunks; ++c) {
           uint32_t v[32];
           tmem_ld32(tAcc + c * 32, v);
           tmem_wait_ld();
-          if (c == D / 32 - 1) {  // the accumulators have left TMEM
+          if (c == kChunks - 1) {  // the accumulators have left TMEM
             tc_fence_before();
             warp_arrive(acc_empty);
           }
-          if (r == 0) {  // the buffer's previous reader (dQ reduce or the store two chunks back)
-            if (c == 0) bulk_wait_group_read<0>(); else bulk_wait_group_read<1>();
+          uint8_t* stg = (kChunks == 4 && c < 2) ? ds_box + c * 8192
+                                                 : dq_stage + (c & 1) * 8192;
+          if (c == 0 || (kChunks == 4 && c == 2)) {
+            if (r == 0) {
+              if (c == 0) bulk_wait_group_read<1>(); else bulk_wait_group_read<2>();
+            }
+            bar_sync(1 + wg, 128);
           }
-          bar_sync(1 + wg, 128);
-          uint8_t* row = stg + (c & 1) * 8192 + r * 64;
+          uint8_t* row = stg + r * 64;
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
             uint4 pk;
@@ -571,7 +589,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           fence_proxy_async_smem();
           bar_sync(1 + wg, 128);
           if (r == 0) {
-            tma_store_3d(wg == 0 ? &tmDK : &tmDV, stg + (c & 1) * 8192, c * 32, g, it.row0);
+            tma_store_3d(wg == 0 ? &tmDK : &tmDV, stg, c * 32, g, it.row0);
             bulk_commit_group();
           }
         }

@@ -1,6 +1,6 @@
 // sched.cuh — device side of the persistent tile scheduler: a scheduler warp of
 // the CTA pulls unit indices from the global atomic cursor, decodes them and hands them to the
-// other warps through a four-slot shared-memory ring, so that every role of a warp-specialised
+// other warps through a small shared-memory ring, so that every role of a warp-specialised
 // kernel walks the same units and the cursor / table latency (several microseconds of dependent
 // L2 round trips) stays off the critical path of short units.
 // The cursor order is the host's longest-first / locality order (worklist.h).
@@ -38,7 +38,7 @@ __device__ __forceinline__ Unit decode_unit(const SchedView& sv, int32_t w, int3
 }
 
 #ifndef BS_SCHED_SLOTS
-#define BS_SCHED_SLOTS 4
+#define BS_SCHED_SLOTS 3
 #endif
 constexpr int kSchedSlots = BS_SCHED_SLOTS;
 
