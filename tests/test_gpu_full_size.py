@@ -1,0 +1,160 @@
+"""-m gpu: BASELINE.json configs 2-5 at FULL size through the C-ABI, in the launch configuration
+bench.py uses (one bs_attn_fwd / bs_attn_bwd per ring step over the whole buffer, bs_lse_merge over
+all steps, prep / finish once).
+
+A full fp64 oracle pass is hours at these sizes, so the comparison is
+  * O, LSE and dQ of a seeded sample of query rows (first / last row of every part, rows next to
+    128-row tile boundaries, random rows), each against the oracle over ALL keys of the sequence -
+    these outputs depend on their own row only, so the sample is exact;
+  * dK, dV of every key row through the O(T) identities that hold for any set of query rows
+    (softmax rows sum to 1, softmax shift invariance):
+        sum_j dV[j,g,:] = sum_{h in g} sum_i dO[i,h,:]        sum_j dK[j,g,:] = 0      per sequence
+    and  sum_i Q_i . dQ_i (heads of g) = sum_j K_j . dK_j      per sequence and KV group.
+"""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+import oracle  # noqa: E402
+from paper_2502_21231_b200 import binding as B  # noqa: E402
+from paper_2502_21231_b200.synth import rng, workloads  # noqa: E402
+
+
+def _sample_rows(pl, n_random, seed, n_boundary=24):
+    """Local Q rows to check: part boundaries, tile boundaries, a few random ones."""
+    cu = pl["cu_rows_q"]
+    rows = set()
+    for a, b in zip(cu[:-1], cu[1:]):
+        if b > a:
+            rows.update([a, b - 1])
+            mid = (a + b) // 2  # for a zigzag shard this is where the high part starts
+            rows.update(x for x in (mid - 1, mid, a + 127, a + 128) if a <= x < b)
+        if len(rows) >= n_boundary:
+            break
+    rows = set(sorted(rows)[:n_boundary])
+    g = np.random.default_rng(seed)
+    rows.update(int(x) for x in g.integers(0, pl["q_rows"], n_random))
+    return np.array(sorted(rows), np.int64)
+
+
+def _run_config(cfg, n_random, n_boundary=24):
+    import gpu_util as U
+    w = workloads.make_workload(cfg)
+    Hq, Hkv, D = w.n_q_heads, w.n_kv_heads, w.head_dim
+    pl = B.plan(w.seqs)
+    opl = oracle.oracle_plan(w.seqs)
+    rows_q, n_steps = pl["q_rows"], pl["n_steps"]
+    qruns = workloads.runs_from(pl["q_seq"], pl["q_pos"])
+    Qb = workloads.gen_rows(w.seed, rng.STREAM_Q, qruns, Hq * D)
+    dOb = workloads.gen_rows(w.seed, rng.STREAM_DO, qruns, Hq * D)
+    Q, dO = U.to_dev(Qb).view(rows_q, Hq, D), U.to_dev(dOb).view(rows_q, Hq, D)
+    # ---------------------------------------------------------------- forward, step by step
+    Kb, Vb, Kd, Vd, parts = [], [], [], [], []
+    for s in range(n_steps):
+        st = pl["steps"][s]
+        kruns = workloads.runs_from(st["k_seq"], st["k_pos"])
+        Kb.append(workloads.gen_rows(w.seed, rng.STREAM_K, kruns, Hkv * D))
+        Vb.append(workloads.gen_rows(w.seed, rng.STREAM_V, kruns, Hkv * D))
+        Kd.append(U.to_dev(Kb[-1]).view(-1, Hkv, D))
+        Vd.append(U.to_dev(Vb[-1]).view(-1, Hkv, D))
+        sh = B.make_shape(Hq, Hkv, D, rows_q, st["kv_rows"])
+        O = torch.empty((rows_q, Hq, D), dtype=torch.bfloat16, device="cuda")
+        L = torch.empty((Hq, rows_q), dtype=torch.float32, device="cuda")
+        ws = torch.empty(B.attn_workspace_bytes(sh, len(st["segs"]), False), dtype=torch.uint8,
+                         device="cuda")
+        B.attn_fwd(sh, Q, Kd[-1], Vd[-1], st["segs"], (0, rows_q), O, L, ws)
+        parts.append((O, L))
+    sh0 = B.make_shape(Hq, Hkv, D, rows_q, pl["steps"][0]["kv_rows"])
+    if n_steps > 1:
+        O = torch.empty_like(parts[0][0])
+        LSE = torch.empty_like(parts[0][1])
+        B.lse_merge([p[0] for p in parts], [p[1] for p in parts], sh0, (0, rows_q), O, LSE)
+    else:
+        O, LSE = parts[0]
+    torch.cuda.synchronize()
+    del parts
+    # ---------------------------------------------------------------- backward
+    delta = torch.empty((Hq, rows_q), dtype=torch.float32, device="cuda")
+    acc = torch.empty((rows_q, Hq, D), dtype=torch.float32, device="cuda")
+    B.attn_bwd_prep(sh0, O, dO, delta, acc)
+    dKs, dVs = [], []
+    for s in range(n_steps):
+        st = pl["steps"][s]
+        sh = B.make_shape(Hq, Hkv, D, rows_q, st["kv_rows"])
+        dK, dV = torch.empty_like(Kd[s]), torch.empty_like(Vd[s])
+        ws = torch.empty(B.attn_workspace_bytes(sh, len(st["segs"]), True), dtype=torch.uint8,
+                         device="cuda")
+        B.attn_bwd(sh, Q, Kd[s], Vd[s], dO, LSE, delta, st["segs"], acc, dK, dV, ws)
+        dKs.append(dK)
+        dVs.append(dV)
+    dQ = torch.empty_like(Q)
+    B.attn_bwd_finish(sh0, acc, dQ)
+    torch.cuda.synchronize()
+    # ---------------------------------------------------------------- sampled rows vs the oracle
+    rows = _sample_rows(pl, n_random, w.seed, n_boundary)
+    ks = np.concatenate([opl["steps"][s]["k_seq"] for s in range(n_steps)])
+    kp = np.concatenate([opl["steps"][s]["k_pos"] for s in range(n_steps)])
+    Kall = np.concatenate(Kb).reshape(-1, Hkv, D)
+    Vall = np.concatenate(Vb).reshape(-1, Hkv, D)
+    qs, qp = opl["q_seq"][rows], opl["q_pos"][rows]
+    Qs, dOs = Qb.reshape(rows_q, Hq, D)[rows], dOb.reshape(rows_q, Hq, D)[rows]
+    Oo, Lo = oracle.attn_fwd(Qs, Kall, Vall, qs, qp, ks, kp)
+    dQo, _, _ = oracle.attn_bwd(Qs, Kall, Vall, dOs, qs, qp, ks, kp)
+    ridx = torch.from_numpy(rows).cuda()
+    got_O = oracle.bf16_to_f64(U.to_bits(O[ridx])).reshape(len(rows), Hq, D)
+    got_L = LSE[:, ridx].double().cpu().numpy()
+    got_dQ = oracle.bf16_to_f64(U.to_bits(dQ[ridx])).reshape(len(rows), Hq, D)
+    diff = np.abs(got_O - Oo)
+    half_ulp = 2.0 ** (np.floor(np.log2(np.maximum(np.abs(Oo), 1e-30))) - 8)
+    tol = np.where(np.abs(Oo) < 4.0, U.TOL_O, half_ulp + 4e-3)  # DESIGN.md reading 19
+    assert np.all(diff <= tol), f"cfg{cfg}: O max abs err {diff.max()} on {len(rows)} sampled rows"
+    err_L = float(np.abs(got_L - Lo).max())
+    assert err_L <= U.TOL_LSE, f"cfg{cfg}: LSE abs err {err_L}"
+    err_dQ = U.rel_l2(got_dQ, dQo)
+    assert err_dQ <= U.TOL_GRAD, f"cfg{cfg}: dQ relative L2 error {err_dQ} on the sample"
+    # ---------------------------------------------------------------- O(T) identities for dK, dV
+    G = Hq // Hkv
+    n_seq = len(w.seqs)
+    qseq = torch.from_numpy(np.ascontiguousarray(pl["q_seq"]).astype(np.int64)).cuda()
+    sum_dO = torch.zeros((n_seq, Hkv, D), dtype=torch.float64, device="cuda")
+    sum_dO.index_add_(0, qseq, dO.double().view(rows_q, Hkv, G, D).sum(2))
+    q_dq = torch.zeros((n_seq, Hkv), dtype=torch.float64, device="cuda")
+    q_dq.index_add_(0, qseq, (Q.double() * dQ.double()).view(rows_q, Hkv, G * D).sum(2))
+    sum_dV = torch.zeros_like(sum_dO)
+    sum_dK = torch.zeros_like(sum_dO)
+    abs_dK = torch.zeros_like(sum_dO)
+    k_dk = torch.zeros_like(q_dq)
+    for s in range(n_steps):
+        kseq = torch.from_numpy(np.ascontiguousarray(pl["steps"][s]["k_seq"]).astype(np.int64)).cuda()
+        sum_dV.index_add_(0, kseq, dVs[s].double())
+        sum_dK.index_add_(0, kseq, dKs[s].double())
+        abs_dK.index_add_(0, kseq, dKs[s].double().abs())
+        k_dk.index_add_(0, kseq, (Kd[s].double() * dKs[s].double()).sum(2))
+    e_dv = float((sum_dV - sum_dO).norm() / sum_dO.norm())
+    e_dk = float(sum_dK.abs().sum() / abs_dK.sum())
+    e_qk = float((q_dq - k_dk).norm() / q_dq.norm())
+    print(f"cfg{cfg}: {len(rows)} sampled rows: O max abs {diff.max():.2e}, LSE {err_L:.1e}, dQ rel-L2 "
+          f"{err_dQ:.1e}; identities: sum dV {e_dv:.1e}, sum dK {e_dk:.1e}, Q.dQ=K.dK {e_qk:.1e}")
+    # bf16 rounding of every dK/dV/dQ element (2^-9 relative, zero mean) is all that separates
+    # the two sides of an identity
+    assert e_dv <= 2e-3, f"cfg{cfg}: sum dV identity off by {e_dv}"
+    assert e_dk <= 2e-3, f"cfg{cfg}: sum dK identity off by {e_dk}"
+    assert e_qk <= 1e-2, f"cfg{cfg}: Q.dQ = K.dK identity off by {e_qk}"
+
+
+def test_cfg2_full_size():
+    _run_config(2, 24)
+
+
+def test_cfg3_full_size():
+    _run_config(3, 6)
+
+
+def test_cfg4_full_size():
+    _run_config(4, 6)
+
+
+def test_cfg5_full_size():
+    _run_config(5, 1, n_boundary=3)  # ~1e11 fp64 flop of oracle per sampled row at 2M keys
