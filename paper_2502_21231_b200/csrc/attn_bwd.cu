@@ -459,37 +459,40 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (r == 0) TRACE(wg, 1, n);
       };
 
-      // dQ of iteration n -> smem -> TMA reduce-add.  In the loop both 32-column chunks go through
-      // this warpgroup's dQ staging tile one after the other (the compute warps have slack there).
-      // After the unit's last iteration (`last`) the dS^T box of this warpgroup is free as well and
-      // takes chunk 0, so the two reduces - and the dK/dV epilogue behind them - do not queue up.
+      // dQ of iteration n -> smem -> TMA reduce-add (fp32 add in L2), 16 columns (one 8 KB box of
+      // 128 rows x 64 B, 64-byte swizzle) at a time.  In the loop the chunks alternate between the
+      // two halves of this warpgroup's dQ staging tile, so a chunk only waits for the reduce two
+      // chunks back to have read its buffer.  After the unit's last iteration (`last`) the dS^T
+      // box of this warpgroup is free as well: four buffers, nothing queues, and the dK/dV
+      // epilogue behind it finds them free in issue order.
       uint8_t* ds_box = smem + L::kDSOff + wg * (kTile * 128);
+      constexpr int kDqChunks = D / 32;  // 16-column chunks of this warpgroup's D/2 columns
       auto drain_dq = [&](uint32_t n, bool last) {
         mbar_wait(dq_full, n & 1);
         if (r == 0) TRACE(wg, 4, n);
         tc_fence_after();
 #pragma unroll
-        for (int c = 0; c < D / 64; ++c) {
-          uint32_t v[32];
-          tmem_ld32(tDQ + c * 32, v);
+        for (int c = 0; c < kDqChunks; ++c) {
+          uint32_t v[16];
+          tmem_ld16(tDQ + c * 16, v);
           tmem_wait_ld();
-          if (c == D / 64 - 1) {
+          if (c == kDqChunks - 1) {
             tc_fence_before();
             warp_arrive(dq_drained);
           }
-          uint8_t* stage = (last && c == 0) ? ds_box : dq_stage;
-          if (r == 0) {  // the previous reader of this staging tile is done
-            if (last) bulk_wait_group_read<1>(); else bulk_wait_group_read<0>();
+          uint8_t* stage = (last ? (c < 2 ? ds_box : dq_stage) : dq_stage) + (c & 1) * 8192;
+          if (r == 0) {  // the previous reader of this buffer is done
+            if (last) bulk_wait_group_read<3>(); else bulk_wait_group_read<1>();
           }
           bar_sync(1 + wg, 128);
 #pragma unroll
-          for (int j = 0; j < 8; ++j)
-            *reinterpret_cast<uint4*>(stage + r * 128 + ((j ^ (r & 7)) * 16)) =
+          for (int j = 0; j < 4; ++j)
+            *reinterpret_cast<uint4*>(stage + r * 64 + ((j ^ ((r >> 1) & 3)) * 16)) =
                 make_uint4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
           fence_proxy_async_smem();
           bar_sync(1 + wg, 128);
           if (r == 0) {
-            tma_reduce_add_3d(&tmDQ, stage, wg * (D / 2) + c * 32, prev_h, prev_qrow);
+            tma_reduce_add_3d(&tmDQ, stage, wg * (D / 2) + c * 16, prev_h, prev_qrow);
             bulk_commit_group();
           }
         }
@@ -556,8 +559,9 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // area (two 8 KB buffers) and out with TMA stores - whole 64-byte row segments, no LSU
         // work.  (Row-per-thread 16-byte global stores cost one half-used sector each: ~5000
         // cycles per unit, measured.)
-        // staging: D = 128: chunks 0,1 in the dS^T box (after the last drain's chunk-0 reduce),
-        // chunks 2,3 in the dQ staging tile (after its chunk-1 reduce); D = 64: the dQ staging tile
+        // staging: the same four 8 KB buffers as the last drain, in the same order (D = 64: the two
+        // dQ staging halves, which that drain did not use); each chunk waits until all but the
+        // three most recent bulk groups have read their source
         constexpr int kChunks = D / 32;
 #pragma unroll
         for (int c = 0; c < kChunks; ++c) {
@@ -568,14 +572,9 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_fence_before();
             warp_arrive(acc_empty);
           }
-          uint8_t* stg = (kChunks == 4 && c < 2) ? ds_box + c * 8192
-                                                 : dq_stage + (c & 1) * 8192;
-          if (c == 0 || (kChunks == 4 && c == 2)) {
-            if (r == 0) {
-              if (c == 0) bulk_wait_group_read<1>(); else bulk_wait_group_read<2>();
-            }
-            bar_sync(1 + wg, 128);
-          }
+          uint8_t* stg = ((kChunks == 4 && c < 2) ? ds_box : dq_stage) + (c & 1) * 8192;
+          if (r == 0) bulk_wait_group_read<3>();
+          bar_sync(1 + wg, 128);
           uint8_t* row = stg + r * 64;
 #pragma unroll
           for (int q = 0; q < 4; ++q) {
@@ -663,26 +662,26 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   const int D = shape->head_dim;
   CUtensorMap tmQ, tmK, tmV, tmDO, tmDQ, tmDK, tmDV;
   rc = bs::make_tensor_map_3d(&tmQ, Q, 2, D, shape->n_q_heads, shape->q_rows, shape->q_row_stride,
-                              64, bs::kTile, true);
+                              64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmDO, dO, 2, D, shape->n_q_heads, shape->q_rows,
-                              shape->q_row_stride, 64, bs::kTile, true);
+                              shape->q_row_stride, 64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmK, K, 2, D, shape->n_kv_heads, shape->kv_rows,
-                              shape->kv_row_stride, 64, bs::kTile, true);
+                              shape->kv_row_stride, 64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmV, V, 2, D, shape->n_kv_heads, shape->kv_rows,
-                              shape->kv_row_stride, 64, bs::kTile, true);
+                              shape->kv_row_stride, 64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmDQ, dQ_acc, 4, D, shape->n_q_heads, shape->q_rows,
-                              (int64_t)shape->n_q_heads * D, 32, bs::kTile, true);
+                              (int64_t)shape->n_q_heads * D, 16, bs::kTile, 64);
   if (rc != BS_OK) return rc;
 
   rc = bs::make_tensor_map_3d(&tmDK, dK, 2, D, shape->n_kv_heads, shape->kv_rows,
-                              shape->kv_row_stride, 32, bs::kTile, false);
+                              shape->kv_row_stride, 32, bs::kTile, 0);
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmDV, dV, 2, D, shape->n_kv_heads, shape->kv_rows,
-                              shape->kv_row_stride, 32, bs::kTile, false);
+                              shape->kv_row_stride, 32, bs::kTile, 0);
   if (rc != BS_OK) return rc;
 
   BwdParams p;

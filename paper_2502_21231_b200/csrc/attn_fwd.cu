@@ -722,13 +722,13 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
   const int D = shape->head_dim;
   CUtensorMap tmQ, tmK, tmV;
   rc = bs::make_tensor_map_3d(&tmQ, Q, 2, D, shape->n_q_heads, shape->q_rows, shape->q_row_stride,
-                              64, bs::kTile, true);
+                              64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmK, K, 2, D, shape->n_kv_heads, shape->kv_rows,
-                              shape->kv_row_stride, 64, bs::kTile, true);
+                              shape->kv_row_stride, 64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmV, V, 2, D, shape->n_kv_heads, shape->kv_rows,
-                              shape->kv_row_stride, 64, bs::kTile, true);
+                              shape->kv_row_stride, 64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
 
   FwdParams p;

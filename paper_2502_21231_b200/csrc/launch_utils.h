@@ -18,11 +18,11 @@ bs_status_t launch_fill_rows(const int2* d_ranges, int n_ranges, int64_t max_row
                              int64_t lse_head_stride, cudaStream_t st);
 
 // 3-D tensor map over a [rows][heads][head_dim] tensor (innermost first: dim, head, row).
-//   elem_bytes 2 (bf16) or 4 (fp32); box = (box_dim, 1, box_rows); swizzle128: 128-byte swizzle
+//   elem_bytes 2 (bf16) or 4 (fp32); box = (box_dim, 1, box_rows); swizzle: 0 (none), 64 or 128 bytes
 //   (box_dim * elem_bytes must be 128) or none.
 bs_status_t make_tensor_map_3d(CUtensorMap* map, const void* base, int elem_bytes, int head_dim,
                                int n_heads, int64_t rows, int64_t row_stride_elems, int box_dim,
-                               int box_rows, bool swizzle128);
+                               int box_rows, int swizzle);
 
 }  // namespace bs
 

@@ -24,7 +24,7 @@ namespace bs {
 
 bs_status_t make_tensor_map_3d(CUtensorMap* map, const void* base, int elem_bytes, int head_dim,
                                int n_heads, int64_t rows, int64_t row_stride_elems, int box_dim,
-                               int box_rows, bool swizzle128) {
+                               int box_rows, int swizzle) {
   std::call_once(g_once, resolve);
   BS_REQUIRE(g_encode != nullptr, BS_ERR_CUDA, "cuTensorMapEncodeTiled unavailable: %s",
              cudaGetErrorString(g_err));
@@ -40,7 +40,8 @@ bs_status_t make_tensor_map_3d(CUtensorMap* map, const void* base, int elem_byte
                                               : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
                         3, const_cast<void*>(base), dims, strides, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE,
-                        swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                        swizzle == 128 ? CU_TENSOR_MAP_SWIZZLE_128B
+                        : swizzle == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   BS_REQUIRE(r == CUDA_SUCCESS, BS_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d",
              (int)r);
