@@ -35,6 +35,10 @@ using namespace bs::ptx;
 
 constexpr int kBwdThreads = 384;
 constexpr int kComputeThreads = 256;
+#ifndef BS_BWD_EMU
+#define BS_BWD_EMU 1
+#endif
+constexpr int kBwdEmuOf4 = BS_BWD_EMU;  // of every 4 column pairs, this many take the FMA-pipe exp2
 
 #ifdef BS_BWD_TRACE
 // debug build only: clock64() stamps of CTA 0: [role][event][iteration]
@@ -58,6 +62,8 @@ struct BwdParams {
   __nv_bfloat16* dK;
   __nv_bfloat16* dV;
   int64_t kv_row_stride;
+  float* dQ_acc;  // [q_rows][Hq][D] fp32 dense
+  int32_t n_q_heads;
 };
 
 template <int D>
@@ -289,13 +295,14 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tma_load_3d(smem + L::kQOff + st * L::kTileBytes + half * (kTile * 128), &tmQ,
                         &q_full[st], half * 64, h, qrow);
         }
-        // lse*log2e (+inf for rows outside the query range: P becomes exactly 0) and delta*scale
+        // -lse*log2e (-inf for rows outside the query range) and -delta*scale
         for (int c = lane; c < kTile; c += 32) {
           const int a = wk.qi * kTile + c;
           const bool ok = a < wk.sp.len;
           const int64_t idx = (int64_t)h * p.lse_head_stride + qrow + c;
-          lse_s[st * kTile + c] = ok ? p.LSE[idx] * 1.4426950408889634f : CUDART_INF_F;
-          delta_s[st * kTile + c] = ok ? p.delta[idx] * p.scale : 0.f;
+          // negated, so that the compute warps fold them in with one packed FMA each
+          lse_s[st * kTile + c] = ok ? -p.LSE[idx] * 1.4426950408889634f : -CUDART_INF_F;
+          delta_s[st * kTile + c] = ok ? -p.delta[idx] * p.scale : 0.f;
         }
         mbar_arrive(&q_full[st]);
         if (lane == 0) {
@@ -421,7 +428,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         continue;
       }
       float P[64];
-      int prev_h = 0, prev_qrow = 0;
+      int prev_h = 0, prev_qrow = 0, prev_qi = 0, prev_len = 0;
       bool first = true;
 
       auto compute_p = [&](const BwdWalker& k, uint32_t n) {
@@ -432,26 +439,29 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tmem_ld32(tS, &s[0]);
         tmem_ld32(tS + 32, &s[32]);
         tmem_wait_ld();
-        const float* lse = lse_s + (n & 1) * kTile + wg * 64;
+        const float2* nl2 = reinterpret_cast<const float2*>(lse_s + (n & 1) * kTile + wg * 64);
         const int a0 = k.qi * kTile + wg * 64;  // query index of this half's first column
-        // column cc visible iff b <= a0 + cc + off
-        const bool full = it.local0 + kTile - 1 <= a0 + k.sp.off && it.local0 + kTile <= it.range_len;
+        // column cc is visible iff c_min <= cc < c_max (key b <= query a0 + cc + off, query inside
+        // its range); `full`: nothing of this warpgroup's 128 x 64 piece is masked (warp-uniform)
+        const bool full = it.local0 + kTile - 1 <= a0 + k.sp.off && it.local0 + kTile <= it.range_len &&
+                          a0 + 64 <= k.sp.len;
         const int c_min = key_ok ? b - k.sp.off - a0 : (1 << 30);
-#pragma unroll
-        for (int c4 = 0; c4 < 16; ++c4) {
-          const float4 l4 = *reinterpret_cast<const float4*>(lse + 4 * c4);
-          const float lv[4] = {l4.x, l4.y, l4.z, l4.w};
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const int cc = 4 * c4 + j;
-            float pv = ex2(fmaf(__uint_as_float(s[cc]), p.scale_log2, -lv[j]));
-            if (!full && cc < c_min) pv = 0.f;
-            P[cc] = pv;
-          }
-        }
+        const int c_max = k.sp.len - a0;
+        const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
         uint32_t pk[32];
 #pragma unroll
-        for (int i = 0; i < 32; ++i) pk[i] = pack_bf16(P[2 * i], P[2 * i + 1]);
+        for (int i = 0; i < 32; ++i) {
+          const float2 x = fma2(make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])),
+                                sc2, nl2[i]);
+          float2 e = (i & 3) < kBwdEmuOf4 ? ex2_fma2(x) : make_float2(ex2(x.x), ex2(x.y));
+          if (!full) {  // masked P exactly 0, whichever exp2 path produced it
+            if (2 * i < c_min || 2 * i >= c_max) e.x = 0.f;
+            if (2 * i + 1 < c_min || 2 * i + 1 >= c_max) e.y = 0.f;
+          }
+          P[2 * i] = e.x;
+          P[2 * i + 1] = e.y;
+          pk[i] = pack_bf16(e.x, e.y);
+        }
         tmem_st32(tP, pk);
         tmem_wait_st();
         tc_fence_before();
@@ -471,15 +481,33 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_wait(dq_full, n & 1);
         if (r == 0) TRACE(wg, 4, n);
         tc_fence_after();
+        // all of this warpgroup's dQ columns into registers first: the TMEM region is handed
+        // back at once, and the MMA issuer's dP^T of the next iteration (same region) does not
+        // wait for the staging below
+        uint32_t vq[D / 2];
+#pragma unroll
+        for (int c = 0; c < D / 64; ++c) tmem_ld32(tDQ + c * 32, &vq[c * 32]);
+        tmem_wait_ld();
+        tc_fence_before();
+        warp_arrive(dq_drained);
+#ifdef BS_BWD_DQ_RED
+        {  // experiment: straight red.global.add.v4.f32 from registers, no staging, no TMA
+          const int a = prev_qi * kTile + r;
+          if (a < prev_len) {
+            float* dst = p.dQ_acc + ((int64_t)(prev_qrow + r) * p.n_q_heads + prev_h) * D + wg * (D / 2);
+#pragma unroll
+            for (int j = 0; j < D / 8; ++j)
+              asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + 4 * j),
+                           "f"(__uint_as_float(vq[4 * j])), "f"(__uint_as_float(vq[4 * j + 1])),
+                           "f"(__uint_as_float(vq[4 * j + 2])), "f"(__uint_as_float(vq[4 * j + 3]))
+                           : "memory");
+          }
+          return;
+        }
+#endif
 #pragma unroll
         for (int c = 0; c < kDqChunks; ++c) {
-          uint32_t v[16];
-          tmem_ld16(tDQ + c * 16, v);
-          tmem_wait_ld();
-          if (c == kDqChunks - 1) {
-            tc_fence_before();
-            warp_arrive(dq_drained);
-          }
+          const uint32_t* v = &vq[c * 16];
           uint8_t* stage = (last ? (c < 2 ? ds_box : dq_stage) : dq_stage) + (c & 1) * 8192;
           if (r == 0) {  // the previous reader of this buffer is done
             if (last) bulk_wait_group_read<3>(); else bulk_wait_group_read<1>();
@@ -492,7 +520,9 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           fence_proxy_async_smem();
           bar_sync(1 + wg, 128);
           if (r == 0) {
+#ifndef BS_BWD_NO_DQ  /* experiment switch: drop the reduce (wrong dQ) to see what it costs */
             tma_reduce_add_3d(&tmDQ, stage, wg * (D / 2) + c * 16, prev_h, prev_qrow);
+#endif
             bulk_commit_group();
           }
         }
@@ -517,22 +547,20 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             if (r == 0) bulk_wait_group_read<0>();
             bar_sync(1 + wg, 128);
           }
-          const float* dl = delta_s + (it_n & 1) * kTile + wg * 64;
+          const float2* nd2 = reinterpret_cast<const float2*>(delta_s + (it_n & 1) * kTile + wg * 64);
+          const float2 s2 = make_float2(p.scale, p.scale);
 #pragma unroll
           for (int j = 0; j < 8; ++j) {  // 8 queries = one 16-byte chunk of the dS^T row
-            const float4 d0 = *reinterpret_cast<const float4*>(dl + 8 * j);
-            const float4 d1 = *reinterpret_cast<const float4*>(dl + 8 * j + 4);
-            const float dv[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
-            float ds[8];
+            uint32_t w4[4];
 #pragma unroll
-            for (int e = 0; e < 8; ++e)
-              ds[e] = P[8 * j + e] * fmaf(__uint_as_float(dp[8 * j + e]), p.scale, -dv[e]);
-            uint4 pk;
-            pk.x = pack_bf16(ds[0], ds[1]);
-            pk.y = pack_bf16(ds[2], ds[3]);
-            pk.z = pack_bf16(ds[4], ds[5]);
-            pk.w = pack_bf16(ds[6], ds[7]);
-            *reinterpret_cast<uint4*>(ds_row + ((j ^ (r & 7)) * 16)) = pk;
+            for (int e = 0; e < 4; ++e) {
+              const int i = 4 * j + e;
+              const float2 t = fma2(make_float2(__uint_as_float(dp[2 * i]), __uint_as_float(dp[2 * i + 1])),
+                                    s2, nd2[i]);
+              const float2 d = mul2(make_float2(P[2 * i], P[2 * i + 1]), t);
+              w4[e] = pack_bf16(d.x, d.y);
+            }
+            *reinterpret_cast<uint4*>(ds_row + ((j ^ (r & 7)) * 16)) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
           }
         }
         fence_proxy_async_smem();
@@ -541,6 +569,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (r == 0) TRACE(wg, 3, it_n);
         prev_h = g * p.group + wk.hi;
         prev_qrow = wk.q_row();
+        prev_qi = wk.qi;
+        prev_len = wk.sp.len;
         first = false;
         ++it_n;
         if (!has_next) break;
@@ -583,7 +613,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             pk.y = pack_bf16(__uint_as_float(v[8 * q + 2]), __uint_as_float(v[8 * q + 3]));
             pk.z = pack_bf16(__uint_as_float(v[8 * q + 4]), __uint_as_float(v[8 * q + 5]));
             pk.w = pack_bf16(__uint_as_float(v[8 * q + 6]), __uint_as_float(v[8 * q + 7]));
-            *reinterpret_cast<uint4*>(row + q * 16) = pk;
+            *reinterpret_cast<uint4*>(row + ((q ^ ((r >> 1) & 3)) * 16)) = pk;  // 64-byte swizzle
           }
           fence_proxy_async_smem();
           bar_sync(1 + wg, 128);
@@ -678,10 +708,10 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   if (rc != BS_OK) return rc;
 
   rc = bs::make_tensor_map_3d(&tmDK, dK, 2, D, shape->n_kv_heads, shape->kv_rows,
-                              shape->kv_row_stride, 32, bs::kTile, 0);
+                              shape->kv_row_stride, 32, bs::kTile, 64);
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmDV, dV, 2, D, shape->n_kv_heads, shape->kv_rows,
-                              shape->kv_row_stride, 32, bs::kTile, 0);
+                              shape->kv_row_stride, 32, bs::kTile, 64);
   if (rc != BS_OK) return rc;
 
   BwdParams p;
@@ -697,6 +727,8 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   p.dK = (__nv_bfloat16*)dK;
   p.dV = (__nv_bfloat16*)dV;
   p.kv_row_stride = shape->kv_row_stride;
+  p.dQ_acc = dQ_acc;
+  p.n_q_heads = shape->n_q_heads;
   const int grid = tb.n_units < bs::sm_count() ? tb.n_units : bs::sm_count();
   if (D == 128) {
     BS_CUDA(cudaFuncSetAttribute(attn_bwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,

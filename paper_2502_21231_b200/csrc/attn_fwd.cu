@@ -40,23 +40,6 @@ constexpr float kRescaleThreshold = 8.f;  // log2 units
 #endif
 constexpr int kEmuOf4 = BS_FWD_EMU;  // of every 4 column pairs, this many take the FMA-pipe exp2
 
-// 2^x for x <= ~8 on the FMA pipe (the MUFU unit is co-critical with the tensor pipe, SURVEY.md
-// 7.2-3): round-to-nearest split x = n + f with the 1.5 * 2^23 trick, degree-3 minimax polynomial
-// of 2^f on [-0.5, 0.5] (relative error 7.5e-5, far below the bf16 rounding of P), n added into
-// the exponent field.  x is clamped at -125, so masked (-inf) scores give ~2^-125 instead of 0.
-__device__ __forceinline__ float2 ex2_fma2(float2 x) {
-  x.x = fmaxf(x.x, -125.f);
-  x.y = fmaxf(x.y, -125.f);
-  const float2 t = add2(x, make_float2(12582912.f, 12582912.f));
-  const float2 n = add2(t, make_float2(-12582912.f, -12582912.f));
-  const float2 f = add2(x, make_float2(-n.x, -n.y));
-  float2 q = fma2(f, make_float2(0.0551716685f, 0.0551716685f), make_float2(0.242611125f, 0.242611125f));
-  q = fma2(q, f, make_float2(0.693260968f, 0.693260968f));
-  q = fma2(q, f, make_float2(0.999928057f, 0.999928057f));
-  return make_float2(__int_as_float(__float_as_int(q.x) + (__float_as_int(t.x) << 23)),
-                     __int_as_float(__float_as_int(q.y) + (__float_as_int(t.y) << 23)));
-}
-
 #ifdef BS_FWD_TRACE
 // debug build only: per-event clock64() stamps of CTA 0 (role, event) x iteration
 __device__ long long g_fwd_trace[4][8][256];
@@ -87,8 +70,8 @@ struct FwdSmem {
   static constexpr int kQOff = 0;                   // 2 Q tiles
   static constexpr int kKVOff = 2 * kTileBytes;     // kStages K/V tiles
   static constexpr int kBarOff = kKVOff + kStages * kTileBytes;
-  // barriers: q_full[2], q_empty[2], kv_full[S], kv_empty[S], s_full[2], p_full[2][2], o_full[2]
-  static constexpr int kNumBars = 4 + 2 * kStages + 8;
+  // barriers: q_full[2], q_empty[2], kv_full[S], kv_empty[S], s_full[2], p_full[2][4], o_full[2]
+  static constexpr int kNumBars = 4 + 2 * kStages + 12;
   static constexpr int kTmemSlotOff = kBarOff + kNumBars * 8;
   static constexpr int kSchedOff = kTmemSlotOff + 16;  // SchedRing of the dynamic scheduler
   static constexpr int kXchOff = kSchedOff + kSchedRingBytes;     // row max [2 tiles][2][2][128], row sum [2][2][128]
@@ -167,18 +150,21 @@ __device__ __forceinline__ void issue_qk(uint32_t tmem_s, uint32_t q_addr, uint3
             idesc, kk > 0);
   }
 }
-// O (+)= P V for keys [64 half, 64 half + 64) of the block
+// O (+)= P V for the 2 x 16 keys of one chunk slot: the softmax threads of both column halves
+// produce their 16-column chunks in the order 3, 0, 1, 2 and hand each over separately, so that
+// the first PV MMAs run under the remaining exponentials.
+__device__ __forceinline__ int chunk_of_slot(int slot) { return (slot + 3) & 3; }
 template <int D>
-__device__ __forceinline__ void issue_pv_half(uint32_t tmem_o, uint32_t tmem_p, uint32_t v_addr,
-                                              int half, bool accumulate) {
+__device__ __forceinline__ void issue_pv_slot(uint32_t tmem_o, uint32_t tmem_p, uint32_t v_addr,
+                                              int slot, bool accumulate) {
   constexpr uint32_t idesc = umma_idesc_bf16(kTile, D, 0, 1);  // B = V is MN-major (d contiguous)
 #pragma unroll
-  for (int k4 = 0; k4 < 4; ++k4) {
-    const int kk = half * 4 + k4;
+  for (int half = 0; half < 2; ++half) {
+    const int kk = half * 4 + chunk_of_slot(slot);
     // 16 keys = 16 rows of 128 B; the second 64-wide d half (D = 128) is one box (16 KB) further
     // P of keys [16 kk, 16 kk + 16) sits over the first 8 columns of its own 16 S columns
     umma_ts(tmem_o, tmem_p + kk * 16, umma_desc_sw128(v_addr + kk * 2048, kTile * 128, 1024), idesc,
-            accumulate || kk > 0);
+            accumulate || half > 0);
   }
 }
 
@@ -210,8 +196,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint64_t* kv_full = bars + 4;
   uint64_t* kv_empty = bars + 4 + kStages;
   uint64_t* s_full = bars + 4 + 2 * kStages;
-  uint64_t* p_full = s_full + 2;  // [tile][half]
-  uint64_t* o_full = p_full + 4;
+  uint64_t* p_full = s_full + 2;  // [tile][chunk slot]
+  uint64_t* o_full = p_full + 8;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kTmemSlotOff);
   SchedRing* sched = reinterpret_cast<SchedRing*>(smem + L::kSchedOff);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -223,8 +209,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       mbar_init(&q_full[t], 1);
       mbar_init(&q_empty[t], 1);
       mbar_init(&s_full[t], 1);
-      mbar_init(&p_full[2 * t], 4);  // one arrival per softmax warp
-      mbar_init(&p_full[2 * t + 1], 4);
+      for (int c = 0; c < 4; ++c) mbar_init(&p_full[4 * t + c], 8);  // one arrival per softmax warp
       mbar_init(&o_full[t], 1);
     }
     for (int i = 0; i < kStages; ++i) {
@@ -368,8 +353,15 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           }
           tc_fence_after();
           if (cur.active(t)) {
-            mbar_wait_spin(&p_full[2 * t], p_ph);      // the two column halves of P
-            mbar_wait_spin(&p_full[2 * t + 1], p_ph);
+            ++n_pv;
+            // the first three chunk slots of P go to the tensor pipe as they arrive, outside the
+            // turn lock (PV MMAs of one tile may interleave freely with the other tile's batch)
+            for (int slot = 0; slot < 3; ++slot) {
+              mbar_wait_spin(&p_full[4 * t + slot], p_ph);
+              tc_fence_after();
+              issue_pv_slot<D>(tO, tS, smem_kv + v_stage * L::kTileBytes, slot, n_pv > 1 || slot > 0);
+            }
+            mbar_wait_spin(&p_full[4 * t + 3], p_ph);
             p_ph ^= 1;
             if (lane == 0) TRACE(2 + t, 0, tr_it);
             tc_fence_after();
@@ -381,10 +373,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           while (atom_cas_shared(turn, 0u, 1u) != 0u) __nanosleep(20);
           if (lane == 0) TRACE(2 + t, 1, tr_it);
           if (cur.active(t)) {
-            ++n_pv;
             {
-              issue_pv_half<D>(tO, tS, smem_kv + v_stage * L::kTileBytes, 0, n_pv > 1);
-              issue_pv_half<D>(tO, tS, smem_kv + v_stage * L::kTileBytes, 1, true);
+              issue_pv_slot<D>(tO, tS, smem_kv + v_stage * L::kTileBytes, 3, true);
               if (n_pv == tot) tc_commit(&o_full[t]);
             }
               if (lane == 0) TRACE(2 + t, 2, tr_it);
@@ -557,20 +547,26 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #else
 #define RELOAD(addr, dst) do {} while (0)  /* experiment only: wrong results */
 #endif
+        auto hand_over = [&](int slot) {  // this warp's chunk of P is in TMEM
+          tmem_wait_st();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&p_full[4 * t + slot]);
+        };
         RELOAD(tS, A);
         exp16(B, 3, lim - 48);
+        hand_over(0);
         tmem_wait_ld();
         RELOAD(tS + 16, B);
         exp16(A, 0, lim);
+        hand_over(1);
         tmem_wait_ld();
         RELOAD(tS + 32, A);
         exp16(B, 1, lim - 16);
+        hand_over(2);
         tmem_wait_ld();
         exp16(A, 2, lim - 32);
-        tmem_wait_st();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&p_full[2 * t + hf]);
+        hand_over(3);
         if (r == 0) TRACE(t, 3 + hf, tr_it);
         ++tr_it;
         ++cnt;

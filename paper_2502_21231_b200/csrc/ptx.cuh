@@ -69,6 +69,23 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) {
       : "l"(reinterpret_cast<uint64_t&>(a)), "l"(reinterpret_cast<uint64_t&>(b)));
   return reinterpret_cast<float2&>(d);
 }
+// 2^x for x <= ~8 on the FMA pipe (the MUFU unit is co-critical with the tensor pipe, SURVEY.md
+// 7.2-3): round-to-nearest split x = n + f with the 1.5 * 2^23 trick, degree-3 minimax polynomial
+// of 2^f on [-0.5, 0.5] (relative error 7.5e-5, far below the bf16 rounding of P), n added into
+// the exponent field.  x is clamped at -125, so masked (-inf) scores give ~2^-125 instead of 0.
+__device__ __forceinline__ float2 ex2_fma2(float2 x) {
+  x.x = fmaxf(x.x, -125.f);
+  x.y = fmaxf(x.y, -125.f);
+  const float2 t = add2(x, make_float2(12582912.f, 12582912.f));
+  const float2 n = add2(t, make_float2(-12582912.f, -12582912.f));
+  const float2 f = add2(x, make_float2(-n.x, -n.y));
+  float2 q = fma2(f, make_float2(0.0551716685f, 0.0551716685f), make_float2(0.242611125f, 0.242611125f));
+  q = fma2(q, f, make_float2(0.693260968f, 0.693260968f));
+  q = fma2(q, f, make_float2(0.999928057f, 0.999928057f));
+  return make_float2(__int_as_float(__float_as_int(q.x) + (__float_as_int(t.x) << 23)),
+                     __int_as_float(__float_as_int(q.y) + (__float_as_int(t.y) << 23)));
+}
+
 // Register reallocation between warpgroups (all warps of the warpgroup must execute it).
 template <int N>
 __device__ __forceinline__ void setmaxnreg_inc() {
