@@ -33,7 +33,8 @@ namespace {
 using namespace bs;
 using namespace bs::ptx;
 
-constexpr int kBwdThreads = 384;
+constexpr int kBwdThreads = 512;   // 2 compute WGs, auxiliary WG (MMA, TMA, scheduler), dQ drain WG
+constexpr int kRegsCompute = 168, kRegsAux = 72, kRegsDrain = 104;  // 2*168 + 72 + 104 = 4*128
 constexpr int kComputeThreads = 256;
 #ifndef BS_BWD_EMU
 #define BS_BWD_EMU 1
@@ -80,7 +81,7 @@ struct BwdSmem {
   static constexpr int kBarOff = kDeltaOff + 2 * kTile * 4;
   // k_full k_empty (+ v_full v_empty at the end) q_full[2] q_empty[2] do_full do_empty s_full p_full dp_full ds_full dq_full
   // dq_drained acc_full acc_empty
-  static constexpr int kNumBars = 18;
+  static constexpr int kNumBars = 19;
   static constexpr int kTmemSlotOff = kBarOff + kNumBars * 8;
   static constexpr int kSchedOff = kTmemSlotOff + 16;
   static constexpr int kBytes = kSchedOff + kSchedRingBytes;
@@ -193,6 +194,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint64_t* k_empty = bars + 1;
   uint64_t* v_full = bars + 16;
   uint64_t* v_empty = bars + 17;
+  uint64_t* dp_loaded = bars + 18;
   uint64_t* q_full = bars + 2;   // [2]
   uint64_t* q_empty = bars + 4;  // [2]
   uint64_t* do_full = bars + 6;
@@ -216,7 +218,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     __trap();
   }
   if (warp == 9 && lane == 0) {
-    sched_ring_init(sched, kComputeThreads + 2);  // compute threads + the MMA lane + the TMA lane
+    sched_ring_init(sched, kComputeThreads + 2 + kTile);  // compute + MMA lane + TMA lane + drain WG
     mbar_init(k_full, 1);
     mbar_init(k_empty, 1);
     mbar_init(v_full, 1);
@@ -232,7 +234,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     mbar_init(dp_full, 1);
     mbar_init(ds_full, kComputeThreads / 32);  // one arrival per compute warp
     mbar_init(dq_full, 1);
-    mbar_init(dq_drained, kComputeThreads / 32);  // one arrival per compute warp
+    mbar_init(dq_drained, 4);  // one arrival per drain warp
+    mbar_init(dp_loaded, kComputeThreads / 32);
     mbar_init(acc_full, 1);
     mbar_init(acc_empty, kComputeThreads / 32);  // one arrival per compute warp
     fence_barrier_init();
@@ -253,6 +256,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   const uint32_t sQ = smem_u32(smem + L::kQOff), sDO = smem_u32(smem + L::kDOOff);
   const uint32_t sDS = smem_u32(smem + L::kDSOff);
 
+  if (warp >= 8 && warp < 12) setmaxnreg_dec<kRegsAux>();
   if (warp == 9) {
     // ============================ TMA producer + LSE/delta staging ============================
     uint32_t item_n = 0, it_n = 0;  // items / iterations issued so far (ring phases)
@@ -362,26 +366,25 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           tc_fence_after();
           TRACE(2, 0, it_n);
           issue_dv<D>(tmem + 384, tmem, sDO, !first);
-          // dP^T = V dO^T (its TMEM region held dQ of the previous iteration)
-          if (!first) {
-            mbar_wait(dq_drained, (it_n - 1) & 1);
-            tc_fence_after();
-          }
-          issue_kmajor<D>(tmem + 128, sV, sDO);
+          // dP^T = V dO^T goes into the S^T / P^T region (in issue order behind dV, which reads
+          // P^T from it); dQ has the second region to itself
+          issue_kmajor<D>(tmem, sV, sDO);
           tc_commit(dp_full);
           tc_commit(do_empty);
           TRACE(2, 1, it_n);
           if (!has_next) tc_commit(v_empty);
-          // S^T of the next iteration (P^T of this one has been consumed by dV, in issue order)
+          // S^T of the next iteration, once the compute warps hold dP^T in registers
           if (has_next) {
             mbar_wait(&q_full[(it_n + 1) & 1], ((it_n + 1) >> 1) & 1);
+            mbar_wait(dp_loaded, it_n & 1);
             tc_fence_after();
             issue_kmajor<D>(tmem, sK, sQ + ((it_n + 1) & 1) * L::kTileBytes);
             tc_commit(s_full);
           }
-          // dK += dS^T Q ; dQ = dS K
+          // dK += dS^T Q ; dQ = dS K (its region was emptied by the drain warpgroup an iteration ago)
           TRACE(2, 2, it_n);
           mbar_wait(ds_full, it_n & 1);
+          if (it_n > 0) mbar_wait(dq_drained, (it_n - 1) & 1);
           TRACE(2, 3, it_n);
           tc_fence_after();
           issue_dk<D>(tmem + 256, sDS, sQ + st * L::kTileBytes, !first);
@@ -399,17 +402,70 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         ++item_n;
       }
     }
+  } else if (warp >= 12) {
+    // ===================================== dQ drain warpgroup =====================================
+    // dQ of every iteration: TMEM -> registers -> shared -> TMA reduce-add (fp32 add in L2) into
+    // dQ_acc, 16 columns (one 8 KB box of 128 rows x 64 B, 64-byte swizzle) at a time through
+    // four staging boxes.  It has the whole next iteration for it: the TMA unit needs ~1300
+    // cycles to read a box, which used to sit on the compute warps' critical path.
+    setmaxnreg_dec<kRegsDrain>();
+    const int r = threadIdx.x & 127;  // query row of the tile
+    const uint32_t tY = tmem + (uint32_t((warp & 3) * 32) << 16) + 128;
+    uint8_t* stage0 = smem + L::kDQOff;
+    uint32_t it_n = 0;
+    UnitConsumer cons{sched};
+    Unit u;
+    while (cons.next(&u)) {
+      const int g = u.head;
+      BwdWalker wk;
+      wk.init(p.sv.spans, u.item, p.group);
+      for (; !wk.done(); wk.next(), ++it_n) {
+        const int h = g * p.group + wk.hi, qrow = wk.q_row();
+        mbar_wait(dq_full, it_n & 1);
+        tc_fence_after();
+#pragma unroll
+        for (int half = 0; half < D / 64; ++half) {
+          uint32_t v[64];
+          tmem_ld32(tY + half * 64, &v[0]);
+          tmem_ld32(tY + half * 64 + 32, &v[32]);
+          tmem_wait_ld();
+          if (half == D / 64 - 1) {  // the region may take dQ of the next iteration
+            tc_fence_before();
+            warp_arrive(dq_drained);
+          }
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            uint8_t* stage = stage0 + c * 8192;
+            if (r == 0) bulk_wait_group_read<3>();  // the reduce four chunks back has read this box
+            bar_sync(3, 128);
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              *reinterpret_cast<uint4*>(stage + r * 64 + ((j ^ ((r >> 1) & 3)) * 16)) =
+                  make_uint4(v[16 * c + 4 * j], v[16 * c + 4 * j + 1], v[16 * c + 4 * j + 2],
+                             v[16 * c + 4 * j + 3]);
+            fence_proxy_async_smem();
+            bar_sync(3, 128);
+            if (r == 0) {
+#ifndef BS_BWD_NO_DQ  /* experiment switch: drop the reduce (wrong dQ) to see what it costs */
+              tma_reduce_add_3d(&tmDQ, stage, half * 64 + c * 16, h, qrow);
+#endif
+              bulk_commit_group();
+            }
+          }
+        }
+      }
+    }
+    if (r == 0) bulk_wait_group<0>();  // all dQ reductions have landed before the CTA exits
   } else if (warp < 8) {
     // ==================================== compute warpgroups ====================================
+    setmaxnreg_inc<kRegsCompute>();
     const int wg = warp >> 2;
     const int r = threadIdx.x & 127;  // key row of the tile
     const uint32_t lane_addr = uint32_t((warp & 3) * 32) << 16;
     const uint32_t tS = tmem + lane_addr + wg * 64;         // this half's S^T columns (fp32)
     const uint32_t tP = tS;                                  // its P^T (packed bf16), 32 columns
-    const uint32_t tDP = tmem + lane_addr + 128 + wg * 64;  // this half's dP^T columns
-    const uint32_t tDQ = tmem + lane_addr + 128 + wg * (D / 2);  // dQ columns drained by this WG
+    const uint32_t tDP = tS;  // dP^T takes the S^T / P^T region over once dV has read P^T
     uint8_t* ds_row = smem + L::kDSOff + wg * (kTile * 128) + r * 128;
-    uint8_t* dq_stage = smem + L::kDQOff + wg * (kTile * 128);
     uint32_t item_n = 0, it_n = 0;
     UnitConsumer cons{sched};
     Unit u;
@@ -428,7 +484,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         continue;
       }
       float P[64];
-      int prev_h = 0, prev_qrow = 0, prev_qi = 0, prev_len = 0;
       bool first = true;
 
       auto compute_p = [&](const BwdWalker& k, uint32_t n) {
@@ -469,71 +524,13 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (r == 0) TRACE(wg, 1, n);
       };
 
-      // dQ of iteration n -> smem -> TMA reduce-add (fp32 add in L2), 16 columns (one 8 KB box of
-      // 128 rows x 64 B, 64-byte swizzle) at a time.  In the loop the chunks alternate between the
-      // two halves of this warpgroup's dQ staging tile, so a chunk only waits for the reduce two
-      // chunks back to have read its buffer.  After the unit's last iteration (`last`) the dS^T
-      // box of this warpgroup is free as well: four buffers, nothing queues, and the dK/dV
-      // epilogue behind it finds them free in issue order.
       uint8_t* ds_box = smem + L::kDSOff + wg * (kTile * 128);
-      constexpr int kDqChunks = D / 32;  // 16-column chunks of this warpgroup's D/2 columns
-      auto drain_dq = [&](uint32_t n, bool last) {
-        mbar_wait(dq_full, n & 1);
-        if (r == 0) TRACE(wg, 4, n);
-        tc_fence_after();
-        // all of this warpgroup's dQ columns into registers first: the TMEM region is handed
-        // back at once, and the MMA issuer's dP^T of the next iteration (same region) does not
-        // wait for the staging below
-        uint32_t vq[D / 2];
-#pragma unroll
-        for (int c = 0; c < D / 64; ++c) tmem_ld32(tDQ + c * 32, &vq[c * 32]);
-        tmem_wait_ld();
-        tc_fence_before();
-        warp_arrive(dq_drained);
-#ifdef BS_BWD_DQ_RED
-        {  // experiment: straight red.global.add.v4.f32 from registers, no staging, no TMA
-          const int a = prev_qi * kTile + r;
-          if (a < prev_len) {
-            float* dst = p.dQ_acc + ((int64_t)(prev_qrow + r) * p.n_q_heads + prev_h) * D + wg * (D / 2);
-#pragma unroll
-            for (int j = 0; j < D / 8; ++j)
-              asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + 4 * j),
-                           "f"(__uint_as_float(vq[4 * j])), "f"(__uint_as_float(vq[4 * j + 1])),
-                           "f"(__uint_as_float(vq[4 * j + 2])), "f"(__uint_as_float(vq[4 * j + 3]))
-                           : "memory");
-          }
-          return;
-        }
-#endif
-#pragma unroll
-        for (int c = 0; c < kDqChunks; ++c) {
-          const uint32_t* v = &vq[c * 16];
-          uint8_t* stage = (last ? (c < 2 ? ds_box : dq_stage) : dq_stage) + (c & 1) * 8192;
-          if (r == 0) {  // the previous reader of this buffer is done
-            if (last) bulk_wait_group_read<3>(); else bulk_wait_group_read<1>();
-          }
-          bar_sync(1 + wg, 128);
-#pragma unroll
-          for (int j = 0; j < 4; ++j)
-            *reinterpret_cast<uint4*>(stage + r * 64 + ((j ^ ((r >> 1) & 3)) * 16)) =
-                make_uint4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
-          fence_proxy_async_smem();
-          bar_sync(1 + wg, 128);
-          if (r == 0) {
-#ifndef BS_BWD_NO_DQ  /* experiment switch: drop the reduce (wrong dQ) to see what it costs */
-            tma_reduce_add_3d(&tmDQ, stage, wg * (D / 2) + c * 16, prev_h, prev_qrow);
-#endif
-            bulk_commit_group();
-          }
-        }
-      };
 
       compute_p(wk, it_n);
       while (true) {
         BwdWalker nxt = wk;
         nxt.next();
         const bool has_next = !nxt.done();
-        if (!first) drain_dq(it_n - 1, false);
         // dS^T = P^T * (dP^T * scale - delta * scale)
         mbar_wait(dp_full, it_n & 1);
         if (r == 0) TRACE(wg, 2, it_n);
@@ -543,6 +540,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           tmem_ld32(tDP, &dp[0]);
           tmem_ld32(tDP + 32, &dp[32]);
           tmem_wait_ld();
+          tc_fence_before();
+          warp_arrive(dp_loaded);  // the region may take S^T of the next iteration
           if (first) {  // the previous unit's last dQ reduce / epilogue stores read this dS^T box
             if (r == 0) bulk_wait_group_read<0>();
             bar_sync(1 + wg, 128);
@@ -567,17 +566,12 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tc_fence_before();
         warp_arrive(ds_full);
         if (r == 0) TRACE(wg, 3, it_n);
-        prev_h = g * p.group + wk.hi;
-        prev_qrow = wk.q_row();
-        prev_qi = wk.qi;
-        prev_len = wk.sp.len;
         first = false;
         ++it_n;
         if (!has_next) break;
         compute_p(nxt, it_n);
         wk = nxt;
       }
-      drain_dq(it_n - 1, true);
       // ------------------------------ epilogue: dK (WG A), dV (WG B) ------------------------------
       if (r == 0) TRACE(wg, 5, it_n - 1);
       mbar_wait(acc_full, item_n & 1);
@@ -589,9 +583,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // area (two 8 KB buffers) and out with TMA stores - whole 64-byte row segments, no LSU
         // work.  (Row-per-thread 16-byte global stores cost one half-used sector each: ~5000
         // cycles per unit, measured.)
-        // staging: the same four 8 KB buffers as the last drain, in the same order (D = 64: the two
-        // dQ staging halves, which that drain did not use); each chunk waits until all but the
-        // three most recent bulk groups have read their source
+        // staging: the two 8 KB halves of this warpgroup's dS^T box (free: the unit's last dK / dQ
+        // MMAs are complete)
         constexpr int kChunks = D / 32;
 #pragma unroll
         for (int c = 0; c < kChunks; ++c) {
@@ -602,8 +595,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_fence_before();
             warp_arrive(acc_empty);
           }
-          uint8_t* stg = ((kChunks == 4 && c < 2) ? ds_box : dq_stage) + (c & 1) * 8192;
-          if (r == 0) bulk_wait_group_read<3>();
+          uint8_t* stg = ds_box + (c & 1) * 8192;
+          if (r == 0) bulk_wait_group_read<1>();  // the store two chunks back has read this buffer
           bar_sync(1 + wg, 128);
           uint8_t* row = stg + r * 64;
 #pragma unroll
