@@ -39,6 +39,21 @@ def peaks():
                 source="fallback (B200_PROFILING.md)")
 
 
+def ncu_traffic(kernel_prefix):
+    """DRAM bytes (read + write) per launch of a kernel from the committed ncu capture
+    (profiles/r01_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum of one
+    `ncu --set full` launch on this workload), or None."""
+    path = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    try:
+        for line in open(path).read().splitlines()[1:]:
+            f = line.split(",")
+            if f[0].startswith(kernel_prefix):
+                return int(f[1]) + int(f[2])
+    except (OSError, ValueError, IndexError):
+        pass
+    return None
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -128,6 +143,7 @@ def run_ours(args, rank, world, local_rank):
     import numpy as np
     import torch
     from paper_2502_21231_b200 import binding as B
+    from paper_2502_21231_b200 import dist_util as DU
     from paper_2502_21231_b200.synth import rng, workloads
 
     torch.cuda.set_device(local_rank)
@@ -137,7 +153,7 @@ def run_ours(args, rank, world, local_rank):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     w = cfg2()
     Hq, Hkv, D = w.n_q_heads, w.n_kv_heads, w.head_dim
-    seed = w.seed + 100 * rank  # same document lengths on every rank, different tensors
+    seed = DU.rank_seed(w.seed, rank)  # same document lengths on every rank, different tensors
     pl = B.plan(w.seqs)
     st = pl["steps"][0]
     rows, pairs = pl["q_rows"], st["visible_pairs"]
@@ -253,10 +269,7 @@ def run_ours(args, rank, world, local_rank):
     ms_e2e = f0.elapsed_time(f1)
     sampler.stop_flag = True
     sampler.join()
-    if dist:
-        t = torch.tensor([ms, ms_e2e], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, ms_e2e = t.tolist()
+    ms, ms_e2e = DU.max_over_ranks(dist, [ms, ms_e2e], "cuda")
     flops_step = 14.0 * D * Hq * pairs
     out = None
     if rank == 0:
@@ -282,7 +295,7 @@ def run_ours(args, rank, world, local_rank):
                            "bwd_tflops": bwd_tflops},
             "roofline": {"kernel": "attn_bwd_kernel<128>", "bound": "tensor", "achieved": bwd_tflops,
                          "peak": pk["tflops"], "unit": "TFLOP/s", "frac": bwd_tflops / pk["tflops"],
-                         "traffic": None},
+                         "traffic": ncu_traffic("attn_bwd_kernel")},
             "merge": merge,
             "cpu_baseline": {"value": fl / dt / 1e12, "unit": "TFLOP/s", "cores": thr, "kind": "oracle",
                              "sample": f"{ORACLE_SAMPLE_HEADS} of {Hq} heads of {WORKLOAD}, all "
@@ -319,7 +332,8 @@ def bench_merge(B, torch, pk):
     gbs = nbytes / (ms * 1e-3) / 1e9
     return {"workload": "cfg3 partials: n=8, 32768 rows, 64 heads, D=128", "ms": ms, "bytes": nbytes,
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s",
-                         "frac": gbs / pk["hbm"], "frac_of_nominal_8000": gbs / 8000.0, "traffic": None}}
+                         "frac": gbs / pk["hbm"], "frac_of_nominal_8000": gbs / 8000.0,
+                         "traffic": ncu_traffic("lse_merge_kernel")}}
 
 
 def main():
