@@ -90,13 +90,14 @@ struct BwdSmem {
 // Iterations of one item: for each query head of the group, for each span (query range), the
 // 128-row query tiles holding at least one query that sees the key tile's first key.
 struct BwdWalker {
-  const Span* spans;
+  const Span* table;
+  const Unit* u;
   int n_spans, group, b0, hi, s, qi, n_qt;
   Span sp;
   __device__ __forceinline__ void load_span() {
     while (hi < group) {
       while (s < n_spans) {
-        sp = spans[s];
+        sp = unit_span(*u, table, s);
         const int a_min = max(0, b0 - sp.off);  // first query that sees key b0
         if (a_min < sp.len) {
           qi = a_min / kTile;
@@ -109,8 +110,10 @@ struct BwdWalker {
       s = 0;
     }
   }
-  __device__ __forceinline__ void init(const Span* table, const Item& it, int g) {
-    spans = table + it.span_begin;
+  __device__ __forceinline__ void init(const Span* sp_table, const Unit& unit, int g) {
+    const Item& it = unit.item;
+    table = sp_table;
+    u = &unit;
     n_spans = it.n_spans;
     group = g;
     b0 = it.local0;
@@ -273,7 +276,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const Item& it = u.item;
       const int g = u.head;
       BwdWalker wk;
-      wk.init(p.sv.spans, it, p.group);
+      wk.init(p.sv.spans, u, p.group);
       if (wk.done()) continue;
       // The first iteration's Q / LSE / delta / dO go out BEFORE this unit's K and V: their
       // buffers free up well before the previous unit ends, whereas V is only released at that
@@ -341,7 +344,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       while (cons.next(&u)) {
         const Item& it = u.item;
         BwdWalker wk;
-        wk.init(p.sv.spans, it, p.group);
+        wk.init(p.sv.spans, u, p.group);
         if (wk.done()) continue;
         mbar_wait(k_full, item_n & 1);
         tc_fence_after();
@@ -418,7 +421,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     while (cons.next(&u)) {
       const int g = u.head;
       BwdWalker wk;
-      wk.init(p.sv.spans, u.item, p.group);
+      wk.init(p.sv.spans, u, p.group);
       for (; !wk.done(); wk.next(), ++it_n) {
         const int h = g * p.group + wk.hi, qrow = wk.q_row();
         mbar_wait(dq_full, it_n & 1);
@@ -475,7 +478,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const int b = it.local0 + r;  // key index inside its range
       const bool key_ok = b < it.range_len;
       BwdWalker wk;
-      wk.init(p.sv.spans, it, p.group);
+      wk.init(p.sv.spans, u, p.group);
       __nv_bfloat16* out = (wg == 0 ? p.dK : p.dV) + ((int64_t)it.row0 + r) * p.kv_row_stride +
                            (int64_t)g * D;
       if (wk.done()) {  // no query sees this key tile: its gradients are zero

@@ -94,14 +94,15 @@ __device__ __forceinline__ int span_blocks(int at0, int rows, const Span& sp) {
 // only: arrays indexed by the runtime tile number would live in local memory.)
 template <bool kUniform>
 struct WalkerT {
-  const Span* spans;
+  const Span* table;
+  const Unit* u;
   int n_spans, s, j, nb0, nb1, at0_1, rows0, rows1;
   Span sp;
   __device__ __forceinline__ int at0(int t) const { return t ? at0_1 : at0_1 - kTile; }
   __device__ __forceinline__ int rows(int t) const { return t ? rows1 : rows0; }
   __device__ __forceinline__ void load_span() {
     while (s < n_spans) {
-      sp = spans[s];
+      sp = unit_span(*u, table, s);
       if (kUniform) {  // converged warp, same span in every lane
         sp.begin = warp_uniform(sp.begin);
         sp.len = warp_uniform(sp.len);
@@ -114,8 +115,10 @@ struct WalkerT {
     }
     j = 0;
   }
-  __device__ __forceinline__ void init(const Span* sp_table, const Item& it) {
-    spans = sp_table + it.span_begin;
+  __device__ __forceinline__ void init(const Span* sp_table, const Unit& unit) {
+    const Item& it = unit.item;
+    table = sp_table;
+    u = &unit;
     n_spans = it.n_spans;
     at0_1 = it.local0 + kTile;
     rows0 = max(0, min(kTile, it.range_len - it.local0));
@@ -134,7 +137,7 @@ struct WalkerT {
   // total blocks tile t takes part in over the whole item
   __device__ __forceinline__ int total(int t) const {
     int n = 0;
-    for (int q = 0; q < n_spans; ++q) n += span_blocks(at0(t), rows(t), spans[q]);
+    for (int q = 0; q < n_spans; ++q) n += span_blocks(at0(t), rows(t), unit_span(*u, table, q));
     return kUniform ? warp_uniform(n) : n;
   }
 };
@@ -242,7 +245,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const Item& it = u.item;
         const int h = u.head, g = h / p.group;
         Walker wk;
-        wk.init(p.sv.spans, it);
+        wk.init(p.sv.spans, u);
         if (wk.done()) continue;
         // Order of a unit's loads: K of the first block (its ring stage is released early, at
         // the S MMAs four stages back), then the two Q tiles (a tile's buffer is released at its
@@ -301,7 +304,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         ++un;
         UTRACE(2 + t, 0, un);
         Walker cur;
-        cur.init(p.sv.spans, u.item);
+        cur.init(p.sv.spans, u);
         if (cur.done()) continue;
         const int tot = cur.total(t);
         UTRACE(2 + t, 1, un);
@@ -418,7 +421,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const Item& it = u.item;
       const int h = u.head;
       Walker wk;
-      wk.init(p.sv.spans, it);
+      wk.init(p.sv.spans, u);
       const int at0 = wk.at0(t);
       const bool valid = r < wk.rows(t);
       const int64_t grow = (int64_t)it.row0 + t * kTile + r;

@@ -21,7 +21,15 @@ struct SchedView {  // device pointers into the uploaded workspace
 struct Unit {
   Item item;
   int32_t head;
+  Span sp[2];  // the item's first two spans (most items have one or two): the consumers' walkers
+               // start from registers instead of a dependent global load at every unit start
 };
+// span s of a unit: cached copy or the global table
+__device__ __forceinline__ Span unit_span(const Unit& u, const Span* table, int s) {
+  if (s == 0) return u.sp[0];
+  if (s == 1) return u.sp[1];
+  return table[u.item.span_begin + s];
+}
 
 // unit index -> (item, head): find the group (a CTA's unit indices only grow, so the search
 // walks forward from the group of its previous unit: *hint), then head-major inside the group.
@@ -34,6 +42,8 @@ __device__ __forceinline__ Unit decode_unit(const SchedView& sv, int32_t w, int3
   Unit u;
   u.head = local / g.n_items;
   u.item = sv.items[g.item_begin + local % g.n_items];
+  u.sp[0] = sv.spans[u.item.span_begin];
+  u.sp[1] = u.item.n_spans > 1 ? sv.spans[u.item.span_begin + 1] : u.sp[0];
   return u;
 }
 
@@ -44,11 +54,12 @@ constexpr int kSchedSlots = BS_SCHED_SLOTS;
 
 struct SchedRing {  // lives in shared memory (16-byte aligned)
   Item item[kSchedSlots];  // decoded by the producer: consumers never touch the global tables
+  Span sp[kSchedSlots][2];
   int32_t head[kSchedSlots];
   int32_t unit[kSchedSlots];
   uint64_t full[kSchedSlots], empty[kSchedSlots];
 };
-constexpr int kSchedRingBytes = 256;
+constexpr int kSchedRingBytes = 384;
 static_assert(sizeof(SchedRing) <= kSchedRingBytes, "SchedRing size");
 
 // n_consumers = arrivals per slot on the empty barrier (threads calling next(), warps calling
@@ -84,6 +95,8 @@ struct UnitProducer {  // one thread (the scheduler warp's lane 0)
     if (w >= 0) {
       r->item[slot] = u->item;
       r->head[slot] = u->head;
+      r->sp[slot][0] = u->sp[0];
+      r->sp[slot][1] = u->sp[1];
     }
     r->unit[slot] = w;
     ptx::mbar_arrive(&r->full[slot]);
@@ -109,6 +122,8 @@ struct UnitConsumer {  // every consuming thread
     if (w >= 0) {
       u->item = r->item[slot];
       u->head = r->head[slot];
+      u->sp[0] = r->sp[slot][0];
+      u->sp[1] = r->sp[slot][1];
     }
     ptx::mbar_arrive(&r->empty[slot]);
     ++n;
@@ -121,6 +136,8 @@ struct UnitConsumer {  // every consuming thread
     ptx::mbar_wait(&r->full[slot], ph);
     u->item = r->item[slot];
     u->head = r->head[slot];
+    u->sp[0] = r->sp[slot][0];
+    u->sp[1] = r->sp[slot][1];
   }
 };
 
