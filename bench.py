@@ -179,10 +179,10 @@ def run_ours(args, rank, world, local_rank):
         p = B.plan(w.seqs)["steps"][0]["segs"]  # a1: host planning is part of the step
         if marks:
             marks[0].record()
-        B.attn_fwd(sh, Q, K, V, p, (0, rows), O, LSE, ws_f)
+        B.attn_fwd(sh, Q, K, V, p, (0, rows), O, LSE, ws_f, acc)  # also clears the dQ accumulator
         if marks:
             marks[1].record()
-        B.attn_bwd_prep(sh, O, dO, delta, acc)
+        B.attn_bwd_prep(sh, O, dO, delta, None)
         if marks:
             marks[2].record()
         B.attn_bwd(sh, Q, K, V, dO, LSE, delta, p, acc, dK, dV, ws_b)
@@ -238,8 +238,8 @@ def run_ours(args, rank, world, local_rank):
             s_run.wait_event(d["in_ready"])
             s_run.wait_event(d["out_done"])     # step i-2's results have left the output buffers
             p = B.plan(w.seqs)["steps"][0]["segs"]
-            B.attn_fwd(sh, d["Q"], d["K"], d["V"], p, (0, rows), d["O"], d["LSE"], d["ws_f"])
-            B.attn_bwd_prep(sh, d["O"], d["dO"], d["delta"], d["acc"])
+            B.attn_fwd(sh, d["Q"], d["K"], d["V"], p, (0, rows), d["O"], d["LSE"], d["ws_f"], d["acc"])
+            B.attn_bwd_prep(sh, d["O"], d["dO"], d["delta"], None)
             B.attn_bwd(sh, d["Q"], d["K"], d["V"], d["dO"], d["LSE"], d["delta"], p, d["acc"], d["dK"],
                        d["dV"], d["ws_b"])
             B.attn_bwd_finish(sh, d["acc"], d["dQ"])

@@ -149,14 +149,20 @@ bs_status_t bs_attn_workspace_bytes(const bs_attn_shape_t* shape, int32_t n_segs
  *   LSE[h,i] = ln sum_j exp(S_ij)   (natural log; -inf if no key is visible)
  *   O[i,h,:] = sum_j exp(S_ij - LSE[h,i]) * V[j, h / (Hq/Hkv), :]   (0 if no key is visible)
  * Rows of the range covered by no segment get O = 0, LSE = -inf.  Rows outside the range are
- * not written.  Q,K,V,O: device bf16.  LSE: device fp32.  segs: host.  ws: device. */
+ * not written.  Q,K,V,O: device bf16.  LSE: device fp32.  segs: host.  ws: device.
+ * dQ_acc_clear (device, fp32 [q_rows][n_q_heads][head_dim] dense, 16-byte aligned, or NULL): if
+ * given, the call also sets rows [out_row_begin, out_row_end) of it to 0 - the zeroing half of
+ * bs_attn_bwd_prep folded into the forward's stores (the forward leaves most of the HBM
+ * bandwidth unused); bs_attn_bwd_prep is then called with dQ_acc = NULL.  With several ring steps
+ * only one forward call of the sequence passes it. */
 bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void* K, const void* V,
                         const bs_seg_t* segs, int32_t n_segs, int32_t out_row_begin,
                         int32_t out_row_end, void* O, float* LSE, void* ws, size_t ws_bytes,
-                        void* stream);
+                        void* stream, float* dQ_acc_clear);
 
 /* Backward preparation (a5): delta[h,i] = sum_d dO[i,h,d] * O_final[i,h,d] for all q_rows, and
- * dQ_acc = 0.  O_final is the MERGED output.  All device pointers. */
+ * dQ_acc = 0 (skipped if dQ_acc is NULL: the accumulator was cleared by bs_attn_fwd).  O_final is
+ * the MERGED output.  All device pointers. */
 bs_status_t bs_attn_bwd_prep(const bs_attn_shape_t* shape, const void* O_final, const void* dO,
                              float* delta, float* dQ_acc, void* stream);
 

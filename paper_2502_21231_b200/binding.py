@@ -75,7 +75,7 @@ lib.bs_plan_destroy.restype = None
 lib.bs_plan_destroy.argtypes = [_vp]
 lib.bs_attn_workspace_bytes.argtypes = [_P(Shape), _i32, ctypes.c_int, _P(_sz)]
 lib.bs_attn_fwd.argtypes = [_P(Shape), _vp, _vp, _vp, _P(Seg), _i32, _i32, _i32, _vp, _vp, _vp,
-                            _sz, _vp]
+                            _sz, _vp, _vp]
 lib.bs_attn_bwd_prep.argtypes = [_P(Shape), _vp, _vp, _vp, _vp, _vp]
 lib.bs_attn_bwd.argtypes = [_P(Shape), _vp, _vp, _vp, _vp, _vp, _vp, _P(Seg), _i32, _vp, _vp, _vp,
                             _vp, _sz, _vp]
@@ -172,16 +172,18 @@ def attn_workspace_bytes(shape, n_segs, bwd):
     return int(out.value)
 
 
-def attn_fwd(shape, Q, K, V, segs, out_rows, O, LSE, ws):
+def attn_fwd(shape, Q, K, V, segs, out_rows, O, LSE, ws, dQ_acc_clear=None):
     sarr, n = make_segs(segs)
     _check(lib.bs_attn_fwd(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), sarr, n, out_rows[0],
                            out_rows[1], _ptr(O), _ptr(LSE), _ptr(ws), ws.numel() * ws.element_size(),
-                           _stream()), "bs_attn_fwd")
+                           _stream(), None if dQ_acc_clear is None else _ptr(dQ_acc_clear)),
+           "bs_attn_fwd")
 
 
 def attn_bwd_prep(shape, O_final, dO, delta, dQ_acc):
     _check(lib.bs_attn_bwd_prep(ctypes.byref(shape), _ptr(O_final), _ptr(dO), _ptr(delta),
-                                _ptr(dQ_acc), _stream()), "bs_attn_bwd_prep")
+                                None if dQ_acc is None else _ptr(dQ_acc), _stream()),
+           "bs_attn_bwd_prep")
 
 
 def attn_bwd(shape, Q, K, V, dO, LSE_final, delta, segs, dQ_acc, dK, dV, ws):

@@ -62,6 +62,7 @@ struct FwdParams {
   __nv_bfloat16* O;
   float* LSE;
   int64_t o_row_stride, lse_head_stride;
+  int32_t clear_acc;  // also zero the fp32 dQ accumulator rows of every unit (TMA stores of zeros)
 };
 
 template <int D>
@@ -76,7 +77,8 @@ struct FwdSmem {
   static constexpr int kSchedOff = kTmemSlotOff + 16;  // SchedRing of the dynamic scheduler
   static constexpr int kXchOff = kSchedOff + kSchedRingBytes;     // row max [2 tiles][2][2][128], row sum [2][2][128]
   static constexpr int kLockOff = kXchOff + 6144;     // turn lock of the two MMA issuers
-  static constexpr int kBytes = kLockOff + 16;
+  static constexpr int kZeroOff = ((kLockOff + 16 + 127) / 128) * 128;  // 8 KB of zeros (TMA source)
+  static constexpr int kBytes = kZeroOff + 8192;
   static constexpr int kAlloc = kBytes + 1024;  // slack to align the base to 1024 B
 };
 
@@ -188,7 +190,8 @@ struct Ring {  // position in the K/V smem ring
 template <int D>
 __global__ void __launch_bounds__(kFwdThreads, 1)
 attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
-                const __grid_constant__ CUtensorMap tmV, const __grid_constant__ FwdParams p) {
+                const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmZ,
+                const __grid_constant__ FwdParams p) {
   using L = FwdSmem<D>;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
@@ -224,6 +227,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     prefetch_tensormap(&tmK);
     prefetch_tensormap(&tmV);
   }
+  if (p.clear_acc) {  // the zero source of the accumulator-clearing stores
+    for (int i = threadIdx.x; i < 8192 / 16; i += blockDim.x)
+      reinterpret_cast<uint4*>(smem + L::kZeroOff)[i] = make_uint4(0, 0, 0, 0);
+    fence_proxy_async_smem();
+  }
   if (warp == kMmaWarp0) tmem_alloc<512>(tmem_slot);
   tc_fence_before();
   __syncthreads();
@@ -244,6 +252,12 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         UTRACE(4, 0, un);
         const Item& it = u.item;
         const int h = u.head, g = h / p.group;
+        if (p.clear_acc) {  // 256 rows x D fp32 of this (unit, head): 64-row x 32-column boxes
+          for (int k = 0; k < 4; ++k)
+            for (int c = 0; c < D / 32; ++c)
+              tma_store_3d(&tmZ, smem + L::kZeroOff, c * 32, h, it.row0 + 64 * k);
+          bulk_commit_group();
+        }
         Walker wk;
         wk.init(p.sv.spans, u);
         if (wk.done()) continue;
@@ -281,6 +295,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
         UTRACE(4, 5, un);
       }
+      if (p.clear_acc) bulk_wait_group<0>();  // the zero stores have landed before the CTA exits
     } else if (warp == kSchedWarp && lane == 0) {
       // ====================================== scheduler ======================================
       UnitProducer prod{sched};
@@ -693,7 +708,7 @@ bs_status_t bs_attn_workspace_bytes(const bs_attn_shape_t* shape, int32_t n_segs
 bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void* K, const void* V,
                         const bs_seg_t* segs, int32_t n_segs, int32_t out_row_begin,
                         int32_t out_row_end, void* O, float* LSE, void* ws, size_t ws_bytes,
-                        void* stream) {
+                        void* stream, float* dQ_acc_clear) {
   bs_status_t rc = bs::validate_shape(shape, "bs_attn_fwd");
   if (rc != BS_OK) return rc;
   BS_REQUIRE(Q && K && V && O && LSE, BS_ERR_INVALID_ARG, "bs_attn_fwd: null tensor pointer");
@@ -702,6 +717,8 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
              BS_ERR_INVALID_ARG, "bs_attn_fwd: output rows [%d,%d) outside [0,%d)", out_row_begin,
              out_row_end, shape->q_rows);
   BS_REQUIRE(((uintptr_t)O & 15) == 0, BS_ERR_INVALID_ARG, "bs_attn_fwd: O not 16-byte aligned");
+  BS_REQUIRE(((uintptr_t)dQ_acc_clear & 15) == 0, BS_ERR_INVALID_ARG,
+             "bs_attn_fwd: dQ_acc_clear not 16-byte aligned");
   if (out_row_end == out_row_begin) return BS_OK;
   cudaStream_t st = (cudaStream_t)stream;
   bs::SchedTables tb;
@@ -716,10 +733,16 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
                             O, nullptr, LSE, shape->n_q_heads, shape->head_dim, shape->q_row_stride,
                             shape->lse_head_stride, st);
   if (rc != BS_OK) return rc;
+  const int D = shape->head_dim;
+  if (dQ_acc_clear != nullptr) {  // rows covered by no unit: cleared here (rare path)
+    const size_t row_bytes = (size_t)shape->n_q_heads * D * sizeof(float);
+    for (const bs::RowRange& f : tb.fill)
+      BS_CUDA(cudaMemsetAsync((uint8_t*)dQ_acc_clear + (size_t)f.begin * row_bytes, 0,
+                              (size_t)(f.end - f.begin) * row_bytes, st));
+  }
   if (tb.items.empty()) return BS_OK;
 
-  const int D = shape->head_dim;
-  CUtensorMap tmQ, tmK, tmV;
+  CUtensorMap tmQ, tmK, tmV, tmZ;
   rc = bs::make_tensor_map_3d(&tmQ, Q, 2, D, shape->n_q_heads, shape->q_rows, shape->q_row_stride,
                               64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
@@ -730,7 +753,13 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
                               shape->kv_row_stride, 64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
 
+  // zero stores: rows clipped at out_row_end by the map itself (a unit's 256 rows may overhang)
+  rc = bs::make_tensor_map_3d(&tmZ, dQ_acc_clear ? (const void*)dQ_acc_clear : Q, 4, D,
+                              shape->n_q_heads, out_row_end, (int64_t)shape->n_q_heads * D, 32, 64, 0);
+  if (rc != BS_OK) return rc;
+
   FwdParams p;
+  p.clear_acc = dQ_acc_clear != nullptr;
   p.sv = bs::make_sched_view(wsb, L, tb, shape->n_q_heads);
   p.n_q_heads = shape->n_q_heads;
   p.group = shape->n_q_heads / shape->n_kv_heads;
@@ -745,11 +774,11 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
   if (D == 128) {
     BS_CUDA(cudaFuncSetAttribute(attn_fwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  FwdSmem<128>::kAlloc));
-    attn_fwd_kernel<128><<<grid, kFwdThreads, FwdSmem<128>::kAlloc, st>>>(tmQ, tmK, tmV, p);
+    attn_fwd_kernel<128><<<grid, kFwdThreads, FwdSmem<128>::kAlloc, st>>>(tmQ, tmK, tmV, tmZ, p);
   } else {
     BS_CUDA(cudaFuncSetAttribute(attn_fwd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  FwdSmem<64>::kAlloc));
-    attn_fwd_kernel<64><<<grid, kFwdThreads, FwdSmem<64>::kAlloc, st>>>(tmQ, tmK, tmV, p);
+    attn_fwd_kernel<64><<<grid, kFwdThreads, FwdSmem<64>::kAlloc, st>>>(tmQ, tmK, tmV, tmZ, p);
   }
   BS_CUDA(cudaGetLastError());
   bs::count_launch();

@@ -159,10 +159,11 @@ __global__ void __launch_bounds__(kStreamThreads) bwd_prep_kernel(const __grid_c
     for (int m = kVecPerHead / 2; m >= 1; m >>= 1) s += __shfl_xor_sync(0xffffffffu, s, m);
     if (valid) {
       if ((c % kVecPerHead) == 0) d_smem[r * p.heads_per_block + h] = s;
-      // zero the fp32 accumulator: 2 float4 per bf16 uint4
-      float4* dq = p.dQ_acc + (((int64_t)(row0 + r) * p.n_heads + h0) * kVecPerHead + c) * 2;
-      dq[0] = make_float4(0.f, 0.f, 0.f, 0.f);
-      dq[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (p.dQ_acc != nullptr) {  // zero the fp32 accumulator: 2 float4 per bf16 uint4
+        float4* dq = p.dQ_acc + (((int64_t)(row0 + r) * p.n_heads + h0) * kVecPerHead + c) * 2;
+        dq[0] = make_float4(0.f, 0.f, 0.f, 0.f);
+        dq[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
     }
   }
   __syncthreads();
@@ -313,7 +314,7 @@ bs_status_t bs_attn_bwd_prep(const bs_attn_shape_t* shape, const void* O_final, 
                              float* delta, float* dQ_acc, void* stream) {
   bs_status_t rc = bs::validate_shape(shape, "bs_attn_bwd_prep");
   if (rc != BS_OK) return rc;
-  BS_REQUIRE(O_final && dO && delta && dQ_acc, BS_ERR_INVALID_ARG, "bs_attn_bwd_prep: null pointer");
+  BS_REQUIRE(O_final && dO && delta, BS_ERR_INVALID_ARG, "bs_attn_bwd_prep: null pointer");
   BS_REQUIRE((((uintptr_t)O_final | (uintptr_t)dO | (uintptr_t)dQ_acc) & 15) == 0,
              BS_ERR_INVALID_ARG, "bs_attn_bwd_prep: pointers must be 16-byte aligned");
   if (shape->q_rows == 0) return BS_OK;

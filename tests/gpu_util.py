@@ -39,8 +39,10 @@ def rel_l2(got, want):
 class DeviceRun:
     """One simulated rank: local Q/dO, per-step K/V, plan from the LIBRARY (bs_plan)."""
 
-    def __init__(self, w, steps=None, gen_kv=True):
+    def __init__(self, w, steps=None, gen_kv=True, fused_clear=False):
         self.w = w
+        self.fused_clear = fused_clear  # dQ_acc cleared by the first bs_attn_fwd instead of prep
+        self.dQ_acc = None
         self.plan = B.plan(w.seqs)
         self.Hq, self.Hkv, self.D = w.n_q_heads, w.n_kv_heads, w.head_dim
         pl = self.plan
@@ -72,6 +74,9 @@ class DeviceRun:
         Returns (O bf16 cuda [q_rows,Hq,D], LSE f32 cuda [Hq,q_rows], per-step partials)."""
         Q = to_dev(self.Q_bits)
         parts = []
+        if self.fused_clear:
+            self.dQ_acc = torch.full((self.q_rows, self.Hq, self.D), float("nan"),
+                                     dtype=torch.float32, device="cuda")
         for s in self.steps:
             st = self.plan["steps"][s]
             sh = self.shape(s)
@@ -82,7 +87,8 @@ class DeviceRun:
                              device="cuda")
             ws = torch.empty(B.attn_workspace_bytes(sh, len(st["segs"]), False), dtype=torch.uint8,
                              device="cuda")
-            B.attn_fwd(sh, Q, K, V, st["segs"], (0, self.q_rows), O, LSE, ws)
+            B.attn_fwd(sh, Q, K, V, st["segs"], (0, self.q_rows), O, LSE, ws,
+                       self.dQ_acc if (self.fused_clear and s == self.steps[0]) else None)
             parts.append((O, LSE))
         torch.cuda.synchronize()
         if len(parts) == 1 or not merge:
@@ -99,9 +105,13 @@ class DeviceRun:
         Q, dO = to_dev(self.Q_bits), to_dev(self.dO_bits)
         sh0 = self.shape(self.steps[0])
         delta = torch.empty((self.Hq, self.q_rows), dtype=torch.float32, device="cuda")
-        dQ_acc = torch.full((self.q_rows, self.Hq, self.D), float("nan"), dtype=torch.float32,
-                            device="cuda")
-        B.attn_bwd_prep(sh0, O, dO, delta, dQ_acc)
+        if self.fused_clear:
+            dQ_acc = self.dQ_acc
+            B.attn_bwd_prep(sh0, O, dO, delta, None)
+        else:
+            dQ_acc = torch.full((self.q_rows, self.Hq, self.D), float("nan"), dtype=torch.float32,
+                                device="cuda")
+            B.attn_bwd_prep(sh0, O, dO, delta, dQ_acc)
         grads = {}
         for s in self.steps:
             st = self.plan["steps"][s]

@@ -40,7 +40,7 @@ def test_validation_without_gpu():
     assert b.attn_workspace_bytes(sh, 3, True) >= 256
     # null pointers are rejected before any launch
     rc = b.lib.bs_attn_fwd(ctypes.byref(sh), None, None, None, None, 0, 0, 10, None, None, None, 0,
-                           None)
+                           None, None)
     assert rc == -1
     rc = b.lib.bs_lse_merge(0, None, None, ctypes.byref(sh), 0, 1, None, None, None)
     assert rc == -1

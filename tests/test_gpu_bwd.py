@@ -8,10 +8,10 @@ pytestmark = pytest.mark.gpu
 from paper_2502_21231_b200.synth.workloads import Workload  # noqa: E402
 
 
-def _run(w):
+def _run(w, fused_clear=False):
     import gpu_util as U
     import oracle
-    run = U.DeviceRun(w)
+    run = U.DeviceRun(w, fused_clear=fused_clear)
     O, LSE, _ = run.forward()
     U.check_forward(run, O, LSE)
     dQ, grads, _ = run.backward(O, LSE)
@@ -46,3 +46,13 @@ def test_zigzag_cp(L, N, r):
 
 def test_mixed_hdp_buffer():
     print(_run(Workload("mixed", 4, 1, 128, [(50, 4, 1), (7, 1, 0), (1200, 2, 0), (300, 1, 0)], 6)))
+
+
+@pytest.mark.parametrize("seqs,Hq,Hkv,D", [
+    ([(129, 1, 0), (255, 1, 0), (257, 1, 0)], 4, 2, 128),       # ragged units overhang into the next document
+    ([(300, 1, 0), (77, 1, 0), (1, 1, 0), (513, 1, 0)], 4, 4, 64),
+    ([(2048, 4, 1)], 4, 2, 128),                                # low part rows see nothing in some steps
+    ([(50, 4, 1), (7, 1, 0), (1200, 2, 0), (300, 1, 0)], 4, 1, 128)])
+def test_accumulator_cleared_by_forward(seqs, Hq, Hkv, D):
+    """dQ_acc (NaN-filled) is cleared by the first step's bs_attn_fwd, prep gets dQ_acc = NULL."""
+    print(_run(Workload("fused", Hq, Hkv, D, seqs, 93), fused_clear=True))

@@ -51,6 +51,7 @@ def _run_config(cfg, n_random, n_boundary=24):
     dOb = workloads.gen_rows(w.seed, rng.STREAM_DO, qruns, Hq * D)
     Q, dO = U.to_dev(Qb).view(rows_q, Hq, D), U.to_dev(dOb).view(rows_q, Hq, D)
     # ---------------------------------------------------------------- forward, step by step
+    acc = torch.full((rows_q, Hq, D), float("nan"), dtype=torch.float32, device="cuda")
     Kb, Vb, Kd, Vd, parts = [], [], [], [], []
     for s in range(n_steps):
         st = pl["steps"][s]
@@ -64,7 +65,8 @@ def _run_config(cfg, n_random, n_boundary=24):
         L = torch.empty((Hq, rows_q), dtype=torch.float32, device="cuda")
         ws = torch.empty(B.attn_workspace_bytes(sh, len(st["segs"]), False), dtype=torch.uint8,
                          device="cuda")
-        B.attn_fwd(sh, Q, Kd[-1], Vd[-1], st["segs"], (0, rows_q), O, L, ws)
+        # as in bench.py: the first step's forward also clears the fp32 dQ accumulator
+        B.attn_fwd(sh, Q, Kd[-1], Vd[-1], st["segs"], (0, rows_q), O, L, ws, acc if s == 0 else None)
         parts.append((O, L))
     sh0 = B.make_shape(Hq, Hkv, D, rows_q, pl["steps"][0]["kv_rows"])
     if n_steps > 1:
@@ -77,8 +79,7 @@ def _run_config(cfg, n_random, n_boundary=24):
     del parts
     # ---------------------------------------------------------------- backward
     delta = torch.empty((Hq, rows_q), dtype=torch.float32, device="cuda")
-    acc = torch.empty((rows_q, Hq, D), dtype=torch.float32, device="cuda")
-    B.attn_bwd_prep(sh0, O, dO, delta, acc)
+    B.attn_bwd_prep(sh0, O, dO, delta, None)
     dKs, dVs = [], []
     for s in range(n_steps):
         st = pl["steps"][s]
