@@ -62,6 +62,7 @@ struct FwdParams {
   __nv_bfloat16* O;
   float* LSE;
   int64_t o_row_stride, lse_head_stride;
+  int32_t wide_stores;  // O rows are 32-byte aligned: 256-bit stores in the epilogue
   int32_t clear_acc;  // also zero the fp32 dQ accumulator rows of every unit (TMA stores of zeros)
 };
 
@@ -607,14 +608,21 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tmem_ld16(tO + c * 16, o);
         tmem_wait_ld();
         if (valid) {
+          uint4 pk[2];
 #pragma unroll
           for (int v = 0; v < 2; ++v) {
-            uint4 pk;
-            pk.x = pack_bf16(__uint_as_float(o[8 * v + 0]) * inv_l, __uint_as_float(o[8 * v + 1]) * inv_l);
-            pk.y = pack_bf16(__uint_as_float(o[8 * v + 2]) * inv_l, __uint_as_float(o[8 * v + 3]) * inv_l);
-            pk.z = pack_bf16(__uint_as_float(o[8 * v + 4]) * inv_l, __uint_as_float(o[8 * v + 5]) * inv_l);
-            pk.w = pack_bf16(__uint_as_float(o[8 * v + 6]) * inv_l, __uint_as_float(o[8 * v + 7]) * inv_l);
-            reinterpret_cast<uint4*>(o_ptr)[c * 2 + v] = pk;
+            pk[v].x = pack_bf16(__uint_as_float(o[8 * v + 0]) * inv_l, __uint_as_float(o[8 * v + 1]) * inv_l);
+            pk[v].y = pack_bf16(__uint_as_float(o[8 * v + 2]) * inv_l, __uint_as_float(o[8 * v + 3]) * inv_l);
+            pk[v].z = pack_bf16(__uint_as_float(o[8 * v + 4]) * inv_l, __uint_as_float(o[8 * v + 5]) * inv_l);
+            pk[v].w = pack_bf16(__uint_as_float(o[8 * v + 6]) * inv_l, __uint_as_float(o[8 * v + 7]) * inv_l);
+          }
+          // row-per-thread stores: one whole 32-byte sector per instruction where the layout
+          // allows (two half-used sectors per 16 columns cost twice the LSU transactions)
+          if (p.wide_stores) {
+            stg256(reinterpret_cast<uint4*>(o_ptr) + c * 2, pk[0], pk[1]);
+          } else {
+            reinterpret_cast<uint4*>(o_ptr)[c * 2] = pk[0];
+            reinterpret_cast<uint4*>(o_ptr)[c * 2 + 1] = pk[1];
           }
         }
       }
@@ -760,6 +768,7 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
 
   FwdParams p;
   p.clear_acc = dQ_acc_clear != nullptr;
+  p.wide_stores = ((uintptr_t)O & 31) == 0 && (shape->q_row_stride * 2) % 32 == 0 && (D * 2) % 32 == 0;
   p.sv = bs::make_sched_view(wsb, L, tb, shape->n_q_heads);
   p.n_q_heads = shape->n_q_heads;
   p.group = shape->n_q_heads / shape->n_kv_heads;

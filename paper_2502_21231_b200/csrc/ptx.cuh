@@ -95,6 +95,12 @@ template <int N>
 __device__ __forceinline__ void setmaxnreg_dec() {
   asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N));
 }
+// 256-bit global store (sm_100: STG.256): one full 32-byte sector per thread; p 32-byte aligned
+__device__ __forceinline__ void stg256(void* p, const uint4& a, const uint4& b) {
+  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(a.x), "r"(a.y), "r"(a.z),
+               "r"(a.w), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w)
+               : "memory");
+}
 // spin-lock primitives on a shared-memory word
 __device__ __forceinline__ uint32_t atom_cas_shared(uint32_t* p, uint32_t cmp, uint32_t val) {
   uint32_t old;
