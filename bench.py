@@ -276,6 +276,7 @@ def run_ours(args, rank, world, local_rank):
         pk = peaks()
         nb = lambda t: t.numel() * t.element_size()  # noqa: E731
         merge = bench_merge(B, torch, pk)
+        ring = bench_ring_steps(B, torch, workloads, pk)
         dt, fl, thr = oracle_sample_run(w, ORACLE_SAMPLE_HEADS)
         bwd_tflops = 10.0 * D * Hq * pairs / (t_bwd * 1e-3) / 1e12
         out = {
@@ -297,6 +298,7 @@ def run_ours(args, rank, world, local_rank):
                          "peak": pk["tflops"], "unit": "TFLOP/s", "frac": bwd_tflops / pk["tflops"],
                          "traffic": ncu_traffic("attn_bwd_kernel")},
             "merge": merge,
+            "ring_steps_cfg3_4_5": ring,
             "cpu_baseline": {"value": fl / dt / 1e12, "unit": "TFLOP/s", "cores": thr, "kind": "oracle",
                              "sample": f"{ORACLE_SAMPLE_HEADS} of {Hq} heads of {WORKLOAD}, all "
                                        f"{rows} tokens, fwd+bwd, fp64, {dt:.1f} s"},
@@ -334,6 +336,56 @@ def bench_merge(B, torch, pk):
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s",
                          "frac": gbs / pk["hbm"], "frac_of_nominal_8000": gbs / 8000.0,
                          "traffic": ncu_traffic("lse_merge_kernel")}}
+
+
+def bench_ring_steps(B, torch, workloads, pk):
+    """Configs 3-5 (GQA long sequences, zigzag CP): one diagonal (step 0) and one off-diagonal
+    (step 1) ring step each, bs_attn_fwd and bs_attn_bwd timed with CUDA events on seeded-shape
+    random device data.  Context for the headline number (which is cfg2): unmasked TFLOP/s."""
+    out = {}
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+
+    def timed(fn, n=3):
+        fn()
+        torch.cuda.synchronize()
+        a, b = ev(), ev()
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
+    for cfg in (3, 4, 5):
+        w = workloads.make_workload(cfg)
+        pl = B.plan(w.seqs)
+        Hq, Hkv, D, rows = w.n_q_heads, w.n_kv_heads, w.head_dim, pl["q_rows"]
+        Q = torch.randn(rows, Hq, D, device="cuda").bfloat16()
+        dO = torch.randn_like(Q)
+        O = torch.empty_like(Q)
+        LSE = torch.full((Hq, rows), 8.0, dtype=torch.float32, device="cuda")
+        delta = torch.zeros_like(LSE)
+        acc = torch.zeros((rows, Hq, D), dtype=torch.float32, device="cuda")
+        for sidx in (0, 1):
+            st = pl["steps"][sidx]
+            kv, segs, pairs = st["kv_rows"], st["segs"], st["visible_pairs"]
+            K = torch.randn(kv, Hkv, D, device="cuda").bfloat16()
+            V = torch.randn_like(K)
+            dK, dV = torch.empty_like(K), torch.empty_like(K)
+            sh = B.make_shape(Hq, Hkv, D, rows, kv)
+            wsf = torch.empty(B.attn_workspace_bytes(sh, len(segs), False), dtype=torch.uint8, device="cuda")
+            wsb = torch.empty(B.attn_workspace_bytes(sh, len(segs), True), dtype=torch.uint8, device="cuda")
+            tf = timed(lambda: B.attn_fwd(sh, Q, K, V, segs, (0, rows), O, LSE, wsf))
+            tb = timed(lambda: B.attn_bwd(sh, Q, K, V, dO, LSE, delta, segs, acc, dK, dV, wsb))
+            f_tf, b_tf = 4.0 * D * Hq * pairs / tf / 1e9, 10.0 * D * Hq * pairs / tb / 1e9
+            both = 14.0 * D * Hq * pairs / (tf + tb) / 1e9
+            out[f"cfg{cfg}_step{sidx}"] = {"fwd_ms": round(tf, 3), "bwd_ms": round(tb, 3),
+                                          "fwd_tflops": round(f_tf, 1), "bwd_tflops": round(b_tf, 1),
+                                          "fwd_bwd_tflops": round(both, 1),
+                                          "frac_of_measured_peak": round(both / pk["tflops"], 3)}
+        del Q, dO, O, LSE, delta, acc
+        torch.cuda.empty_cache()
+    return out
 
 
 def main():
