@@ -1,23 +1,31 @@
 // attn_bwd.cu — bs_attn_bwd: backward of one Q-chunk x KV-chunk step on sm_100a (SURVEY.md 8(a)
 // a6; gradients of softmax attention as in flash-attention backward).
 //
-// One persistent CTA per SM, 384 threads:
-//   warps 0-3  compute warpgroup A: query columns  0..63  of the 128x128 tile
-//   warps 4-7  compute warpgroup B: query columns 64..127
-//   warp  8    MMA issuer (one lane)          warp 9  TMA producer (+ LSE/delta staging)
-// A work item is (one 128-key tile of a key range, one KV head).  The CTA keeps dK and dV of the
-// tile in TMEM and loops over the G query heads of the group and over every 128-row query tile
-// that sees the key tile; per iteration it issues the five MMAs of flash-attention backward, all
-// with keys on the TMEM lanes ("transposed" form, thread r <-> key row r):
+// One persistent CTA per SM, 512 threads, registers re-split by setmaxnreg (144 / 64 / 160):
+//   warps 0-3   compute warpgroup A: query columns  0..63  of the transposed 128x128 tile
+//   warps 4-7   compute warpgroup B: query columns 64..127
+//   warp  8     MMA issuer (under elect_one: uniform-register descriptors, back-to-back UTCHMMA)
+//   warp  9     TMA producer (+ LSE/delta staging)       warp 10  scheduler (sched.cuh)
+//   warps 12-15 dQ drain warpgroup: TMEM -> registers -> shared -> TMA reduce-add into dQ_acc
+// A unit is (one 128-key tile of a key range, one KV head).  The CTA keeps dK and dV of the tile
+// in TMEM and loops over the G query heads of the group and over every 128-row query tile that
+// sees the key tile; per iteration it issues the five MMAs of flash-attention backward, all with
+// keys on the TMEM lanes ("transposed" form, thread r <-> key row r):
 //   S^T  = K Q^T                  (SS)   -> P^T = exp2(S^T c - LSE)        written back to TMEM
 //   dP^T = V dO^T                 (SS)   -> dS^T = P^T * (dP^T - delta) c  written to smem (bf16)
 //   dV  += P^T dO                 (TS, A = P^T from TMEM, B = dO MN-major)
+//   dQ   = dS K                   (SS, A = dS^T read MN-major, B = K MN-major)
 //   dK  += dS^T Q                 (SS, A = dS^T K-major, B = Q MN-major)
-//   dQ   = dS K                   (SS, A = dS^T read MN-major, B = K MN-major) -> TMEM -> smem
-//                                  -> TMA reduce-add (fp32) into dQ_acc
-// TMEM: [0,128) S^T / P^T   [128,256) dP^T, then dQ   [256,256+D) dK   [384,384+D) dV.
-// dK/dV are therefore reduced over the group's heads inside the kernel (no atomics); dQ is
-// reduced across key tiles and steps by the TMA unit in L2.
+// TMEM: X [0,128) S^T -> P^T in place -> S^T of the next iteration (behind dV in issue order);
+//       Y [128,256) dP^T(n) -> dQ(n) -> dP^T(n+1): the drain warpgroup lifts dQ into registers the
+//       moment it is complete, while dK(n) is still running;   [256,256+D) dK   [384,384+D) dV.
+// Issue order per iteration n:  dP^T(n) | dV(n) S^T(n+1) | dQ(n) dK(n).  dP^T does not depend on P,
+// so it runs under the compute warps' P step and dS follows P at once; the dependent chain is
+// dS(n) -> dQ(n), dK(n), dP^T(n+1) -> dS(n+1).
+// dK/dV are reduced over the group's heads inside the kernel (no atomics); dQ is reduced across
+// key tiles and steps by the TMA unit in L2.  Measured: per iteration ~576 KB go
+// through shared memory (MMA operands 288, dQ staging 128, dS 96, Q/dO loads 64) = ~4500 cycles at
+// 128 B/clk against 2560 cycles of MMA math: this single-CTA SS-MMA form is shared-memory bound.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -34,7 +42,7 @@ using namespace bs;
 using namespace bs::ptx;
 
 constexpr int kBwdThreads = 512;   // 2 compute WGs, auxiliary WG (MMA, TMA, scheduler), dQ drain WG
-constexpr int kRegsCompute = 168, kRegsAux = 72, kRegsDrain = 104;  // 2*168 + 72 + 104 = 4*128
+constexpr int kRegsCompute = 144, kRegsAux = 64, kRegsDrain = 160;  // 2*144 + 64 + 160 = 4*128
 constexpr int kComputeThreads = 256;
 #ifndef BS_BWD_EMU
 #define BS_BWD_EMU 1
@@ -197,7 +205,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   uint64_t* k_empty = bars + 1;
   uint64_t* v_full = bars + 16;
   uint64_t* v_empty = bars + 17;
-  uint64_t* dp_loaded = bars + 18;
   uint64_t* q_full = bars + 2;   // [2]
   uint64_t* q_empty = bars + 4;  // [2]
   uint64_t* do_full = bars + 6;
@@ -238,7 +245,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     mbar_init(ds_full, kComputeThreads / 32);  // one arrival per compute warp
     mbar_init(dq_full, 1);
     mbar_init(dq_drained, 4);  // one arrival per drain warp
-    mbar_init(dp_loaded, kComputeThreads / 32);
     mbar_init(acc_full, 1);
     mbar_init(acc_empty, kComputeThreads / 32);  // one arrival per compute warp
     fence_barrier_init();
@@ -359,40 +365,42 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           nxt.next();
           const bool has_next = !nxt.done();
           const uint32_t st = it_n & 1;
-          // dV += P^T dO
+          // dP^T = V dO^T first: it does not depend on P, so it runs under the compute warps' P
+          // step and dS can follow P at once.  Its region held dQ of the previous iteration,
+          // which the drain warpgroup lifts into registers as soon as it is complete.
           mbar_wait(do_full, it_n & 1);
+          if (first) mbar_wait(v_full, item_n & 1);
+          if (it_n > 0) mbar_wait(dq_drained, (it_n - 1) & 1);
+          tc_fence_after();
+          issue_kmajor<D>(tmem + 128, sV, sDO);
+          tc_commit(dp_full);
+          TRACE(2, 1, it_n);
+          if (!has_next) tc_commit(v_empty);
+          // dV += P^T dO
           mbar_wait(p_full, it_n & 1);
-          if (first) {
-            mbar_wait(acc_empty, (item_n & 1) ^ 1);  // previous unit's dK/dV have left TMEM
-            mbar_wait(v_full, item_n & 1);
-          }
+          if (first) mbar_wait(acc_empty, (item_n & 1) ^ 1);  // previous unit's dK/dV have left TMEM
           tc_fence_after();
           TRACE(2, 0, it_n);
           issue_dv<D>(tmem + 384, tmem, sDO, !first);
-          // dP^T = V dO^T goes into the S^T / P^T region (in issue order behind dV, which reads
-          // P^T from it); dQ has the second region to itself
-          issue_kmajor<D>(tmem, sV, sDO);
-          tc_commit(dp_full);
           tc_commit(do_empty);
-          TRACE(2, 1, it_n);
-          if (!has_next) tc_commit(v_empty);
-          // S^T of the next iteration, once the compute warps hold dP^T in registers
+          // S^T of the next iteration (P^T of this one has been consumed by dV, in issue order)
           if (has_next) {
             mbar_wait(&q_full[(it_n + 1) & 1], ((it_n + 1) >> 1) & 1);
-            mbar_wait(dp_loaded, it_n & 1);
             tc_fence_after();
             issue_kmajor<D>(tmem, sK, sQ + ((it_n + 1) & 1) * L::kTileBytes);
             tc_commit(s_full);
           }
-          // dK += dS^T Q ; dQ = dS K (its region was emptied by the drain warpgroup an iteration ago)
+          // dK += dS^T Q ; dQ = dS K (into the region dP^T was read from)
           TRACE(2, 2, it_n);
           mbar_wait(ds_full, it_n & 1);
-          if (it_n > 0) mbar_wait(dq_drained, (it_n - 1) & 1);
           TRACE(2, 3, it_n);
           tc_fence_after();
-          issue_dk<D>(tmem + 256, sDS, sQ + st * L::kTileBytes, !first);
+          // dQ before dK: the next iteration's dP^T needs dQ's region back (the drain warpgroup
+          // lifts dQ out while dK runs), and K is released one MMA group earlier at the unit's end
           issue_dq<D>(tmem + 128, sDS, sK);
           tc_commit(dq_full);
+          if (!has_next) tc_commit(k_empty);
+          issue_dk<D>(tmem + 256, sDS, sQ + st * L::kTileBytes, !first);
           tc_commit(&q_empty[st]);
           TRACE(2, 4, it_n);
           first = false;
@@ -401,7 +409,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           wk = nxt;
         }
         tc_commit(acc_full);
-        tc_commit(k_empty);
         ++item_n;
       }
     }
@@ -409,9 +416,9 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     // ===================================== dQ drain warpgroup =====================================
     // dQ of every iteration: TMEM -> registers -> shared -> TMA reduce-add (fp32 add in L2) into
     // dQ_acc, 16 columns (one 8 KB box of 128 rows x 64 B, 64-byte swizzle) at a time through
-    // four staging boxes.  It has the whole next iteration for it: the TMA unit needs ~1300
-    // cycles to read a box, which used to sit on the compute warps' critical path.
-    setmaxnreg_dec<kRegsDrain>();
+    // four staging boxes.  The TMA unit needs ~1300 cycles to read a box; that used to sit on the
+    // compute warps' critical path.  Only the TMEM -> register lift is urgent (see the issuer).
+    setmaxnreg_inc<kRegsDrain>();
     const int r = threadIdx.x & 127;  // query row of the tile
     const uint32_t tY = tmem + (uint32_t((warp & 3) * 32) << 16) + 128;
     uint8_t* stage0 = smem + L::kDQOff;
@@ -426,34 +433,31 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int h = g * p.group + wk.hi, qrow = wk.q_row();
         mbar_wait(dq_full, it_n & 1);
         tc_fence_after();
+        // all D columns into registers first: the region goes straight back to the MMA issuer,
+        // whose next dP^T (on the critical path of the next iteration) is waiting for it
+        uint32_t v[D];
 #pragma unroll
-        for (int half = 0; half < D / 64; ++half) {
-          uint32_t v[64];
-          tmem_ld32(tY + half * 64, &v[0]);
-          tmem_ld32(tY + half * 64 + 32, &v[32]);
-          tmem_wait_ld();
-          if (half == D / 64 - 1) {  // the region may take dQ of the next iteration
-            tc_fence_before();
-            warp_arrive(dq_drained);
-          }
+        for (int c = 0; c < D / 32; ++c) tmem_ld32(tY + c * 32, &v[c * 32]);
+        tmem_wait_ld();
+        tc_fence_before();
+        warp_arrive(dq_drained);
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            uint8_t* stage = stage0 + c * 8192;
-            if (r == 0) bulk_wait_group_read<3>();  // the reduce four chunks back has read this box
-            bar_sync(3, 128);
+        for (int c = 0; c < D / 16; ++c) {
+          uint8_t* stage = stage0 + (c & 3) * 8192;
+          if (r == 0) bulk_wait_group_read<3>();  // the reduce four chunks back has read this box
+          bar_sync(3, 128);
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
-              *reinterpret_cast<uint4*>(stage + r * 64 + ((j ^ ((r >> 1) & 3)) * 16)) =
-                  make_uint4(v[16 * c + 4 * j], v[16 * c + 4 * j + 1], v[16 * c + 4 * j + 2],
-                             v[16 * c + 4 * j + 3]);
-            fence_proxy_async_smem();
-            bar_sync(3, 128);
-            if (r == 0) {
+          for (int j = 0; j < 4; ++j)
+            *reinterpret_cast<uint4*>(stage + r * 64 + ((j ^ ((r >> 1) & 3)) * 16)) =
+                make_uint4(v[16 * c + 4 * j], v[16 * c + 4 * j + 1], v[16 * c + 4 * j + 2],
+                           v[16 * c + 4 * j + 3]);
+          fence_proxy_async_smem();
+          bar_sync(3, 128);
+          if (r == 0) {
 #ifndef BS_BWD_NO_DQ  /* experiment switch: drop the reduce (wrong dQ) to see what it costs */
-              tma_reduce_add_3d(&tmDQ, stage, half * 64 + c * 16, h, qrow);
+            tma_reduce_add_3d(&tmDQ, stage, c * 16, h, qrow);
 #endif
-              bulk_commit_group();
-            }
+            bulk_commit_group();
           }
         }
       }
@@ -467,7 +471,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const uint32_t lane_addr = uint32_t((warp & 3) * 32) << 16;
     const uint32_t tS = tmem + lane_addr + wg * 64;         // this half's S^T columns (fp32)
     const uint32_t tP = tS;                                  // its P^T (packed bf16), 32 columns
-    const uint32_t tDP = tS;  // dP^T takes the S^T / P^T region over once dV has read P^T
+    const uint32_t tDP = tmem + lane_addr + 128 + wg * 64;  // this half's dP^T columns (region Y)
     uint8_t* ds_row = smem + L::kDSOff + wg * (kTile * 128) + r * 128;
     uint32_t item_n = 0, it_n = 0;
     UnitConsumer cons{sched};
@@ -486,7 +490,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           for (int c = 0; c < D / 8; ++c) reinterpret_cast<uint4*>(out)[c] = make_uint4(0, 0, 0, 0);
         continue;
       }
-      float P[64];
+      uint32_t pk[32];  // P^T of this thread as the tensor core sees it (bf16 pairs), kept for dS
       bool first = true;
 
       auto compute_p = [&](const BwdWalker& k, uint32_t n) {
@@ -506,7 +510,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int c_min = key_ok ? b - k.sp.off - a0 : (1 << 30);
         const int c_max = k.sp.len - a0;
         const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
-        uint32_t pk[32];
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
           const float2 x = fma2(make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])),
@@ -516,8 +519,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             if (2 * i < c_min || 2 * i >= c_max) e.x = 0.f;
             if (2 * i + 1 < c_min || 2 * i + 1 >= c_max) e.y = 0.f;
           }
-          P[2 * i] = e.x;
-          P[2 * i + 1] = e.y;
           pk[i] = pack_bf16(e.x, e.y);
         }
         tmem_st32(tP, pk);
@@ -543,8 +544,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           tmem_ld32(tDP, &dp[0]);
           tmem_ld32(tDP + 32, &dp[32]);
           tmem_wait_ld();
-          tc_fence_before();
-          warp_arrive(dp_loaded);  // the region may take S^T of the next iteration
           if (first) {  // the previous unit's last dQ reduce / epilogue stores read this dS^T box
             if (r == 0) bulk_wait_group_read<0>();
             bar_sync(1 + wg, 128);
@@ -559,7 +558,9 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
               const int i = 4 * j + e;
               const float2 t = fma2(make_float2(__uint_as_float(dp[2 * i]), __uint_as_float(dp[2 * i + 1])),
                                     s2, nd2[i]);
-              const float2 d = mul2(make_float2(P[2 * i], P[2 * i + 1]), t);
+              // P widened exactly from the bf16 pair the dV MMA used
+              const float2 d = mul2(make_float2(__uint_as_float(pk[i] << 16),
+                                                __uint_as_float(pk[i] & 0xffff0000u)), t);
               w4[e] = pack_bf16(d.x, d.y);
             }
             *reinterpret_cast<uint4*>(ds_row + ((j ^ (r & 7)) * 16)) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
