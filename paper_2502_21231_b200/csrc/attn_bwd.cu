@@ -454,9 +454,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           fence_proxy_async_smem();
           bar_sync(3, 128);
           if (r == 0) {
-#ifndef BS_BWD_NO_DQ  /* experiment switch: drop the reduce (wrong dQ) to see what it costs */
             tma_reduce_add_3d(&tmDQ, stage, c * 16, h, qrow);
-#endif
             bulk_commit_group();
           }
         }
