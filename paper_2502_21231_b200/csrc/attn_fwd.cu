@@ -561,11 +561,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           if (edge) __syncwarp();
           tmem_st8(tS + 16 * k, pk);
         };
-#if !defined(BS_FWD_NORELOAD) && !(defined(BS_FWD_EXPERIMENT) && BS_FWD_EXPERIMENT == 2)
 #define RELOAD(addr, dst) tmem_ld16(addr, reinterpret_cast<uint32_t*>(dst))
-#else
-#define RELOAD(addr, dst) do {} while (0)  /* experiment only: wrong results */
-#endif
         auto hand_over = [&](int slot) {  // this warp's chunk of P is in TMEM
           tmem_wait_st();
           tc_fence_before();
