@@ -542,6 +542,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           tmem_ld32(tDP, &dp[0]);
           tmem_ld32(tDP + 32, &dp[32]);
           tmem_wait_ld();
+          if (r == 0) TRACE(wg, 8, it_n);
           if (first) {  // the previous unit's last dQ reduce / epilogue stores read this dS^T box
             if (r == 0) bulk_wait_group_read<0>();
             bar_sync(1 + wg, 128);
@@ -564,6 +565,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             *reinterpret_cast<uint4*>(ds_row + ((j ^ (r & 7)) * 16)) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
           }
         }
+        if (r == 0) TRACE(wg, 9, it_n);
         fence_proxy_async_smem();
         tc_fence_before();
         warp_arrive(ds_full);
