@@ -32,6 +32,7 @@
 
 #include "common.h"
 #include "launch_utils.h"
+#include <type_traits>
 #include "ptx.cuh"
 #include "sched.cuh"
 #include "worklist.h"
@@ -508,17 +509,22 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int c_min = key_ok ? b - k.sp.off - a0 : (1 << 30);
         const int c_max = k.sp.len - a0;
         const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
+        // two copies of the loop: unmasked pieces (nearly all of them) run branch- and
+        // predicate-free straight-line code
+        auto exp_all = [&](auto masked) {
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          const float2 x = fma2(make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])),
-                                sc2, nl2[i]);
-          float2 e = (i & 3) < kBwdEmuOf4 ? ex2_fma2(x) : make_float2(ex2(x.x), ex2(x.y));
-          if (!full) {  // masked P exactly 0, whichever exp2 path produced it
-            if (2 * i < c_min || 2 * i >= c_max) e.x = 0.f;
-            if (2 * i + 1 < c_min || 2 * i + 1 >= c_max) e.y = 0.f;
+          for (int i = 0; i < 32; ++i) {
+            const float2 x = fma2(make_float2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])),
+                                  sc2, nl2[i]);
+            float2 e = (i & 3) < kBwdEmuOf4 ? ex2_fma2(x) : make_float2(ex2(x.x), ex2(x.y));
+            if (decltype(masked)::value) {  // masked P exactly 0, whichever exp2 path produced it
+              if (2 * i < c_min || 2 * i >= c_max) e.x = 0.f;
+              if (2 * i + 1 < c_min || 2 * i + 1 >= c_max) e.y = 0.f;
+            }
+            pk[i] = pack_bf16(e.x, e.y);
           }
-          pk[i] = pack_bf16(e.x, e.y);
-        }
+        };
+        if (full) exp_all(std::false_type{}); else exp_all(std::true_type{});
         tmem_st32(tP, pk);
         tmem_wait_st();
         tc_fence_before();
@@ -528,8 +534,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
       uint8_t* ds_box = smem + L::kDSOff + wg * (kTile * 128);
 
-      compute_p(wk, it_n);
       while (true) {
+        compute_p(wk, it_n);
         BwdWalker nxt = wk;
         nxt.next();
         const bool has_next = !nxt.done();
@@ -573,7 +579,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         first = false;
         ++it_n;
         if (!has_next) break;
-        compute_p(nxt, it_n);
         wk = nxt;
       }
       // ------------------------------ epilogue: dK (WG A), dV (WG B) ------------------------------

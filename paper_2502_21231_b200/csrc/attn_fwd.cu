@@ -157,9 +157,9 @@ __device__ __forceinline__ void issue_qk(uint32_t tmem_s, uint32_t q_addr, uint3
   }
 }
 // O (+)= P V for the 2 x 16 keys of one chunk slot: the softmax threads of both column halves
-// produce their 16-column chunks in the order 3, 0, 1, 2 and hand each over separately, so that
+// produce their 16-column chunks in the order 3, 2, 0, 1 and hand each over separately, so that
 // the first PV MMAs run under the remaining exponentials.
-__device__ __forceinline__ int chunk_of_slot(int slot) { return (slot + 3) & 3; }
+__device__ __forceinline__ int chunk_of_slot(int slot) { return (0x3201 >> (4 * (3 - slot))) & 3; }
 template <int D>
 __device__ __forceinline__ void issue_pv_slot(uint32_t tmem_o, uint32_t tmem_p, uint32_t v_addr,
                                               int slot, bool accumulate) {
@@ -462,10 +462,15 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tc_fence_after();
         // Two passes over this thread's 64 columns in chunks of 16, double-buffered in A / B so
         // that the TMEM load of the next chunk runs under the arithmetic of the current one.
-        // Pass 1: row maximum.  Pass 2 (chunks 3, 0, 1, 2; chunk 3 is still in B): P = 2^(S c - m),
+        // Pass 1: row maximum.  Pass 2 (chunks 3, 2, 0, 1; chunk 3 is still in B): P = 2^(S c - m),
         // packed to bf16 and written over the chunk's own first 8 columns.
         const int b0 = wk.j * kTile;
-        const bool edge = b0 + kTile - 1 > at0 + wk.sp.off || b0 + kTile > wk.sp.len;
+        const bool edge_block = b0 + kTile - 1 > at0 + wk.sp.off || b0 + kTile > wk.sp.len;
+        // The block body exists twice: interior blocks (all columns visible) run branch-free
+        // straight-line code (the instruction fetch of a warp that jumps over the masking code
+        // of every chunk costs 8 % of the kernel), blocks on a mask boundary the general one.
+        auto softmax_block = [&](auto edge_c) {
+        constexpr bool edge = decltype(edge_c)::value;
         // last visible column of this row relative to this thread's first column (>= 63: all)
         const int lim = edge ? min(at0 + r + wk.sp.off, wk.sp.len - 1) - b0 - hf * 64 : 64;
         float A[16], B[16];
@@ -491,16 +496,14 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           }
         };
         tmem_ld16(tS, reinterpret_cast<uint32_t*>(A));
-        tmem_wait_ld();
         tmem_ld16(tS + 16, reinterpret_cast<uint32_t*>(B));
-        max16m(A, lim);
         tmem_wait_ld();
+        max16m(A, lim);
         tmem_ld16(tS + 32, reinterpret_cast<uint32_t*>(A));
         max16m(B, lim - 16);
-        tmem_wait_ld();
         tmem_ld16(tS + 48, reinterpret_cast<uint32_t*>(B));
-        max16m(A, lim - 32);
         tmem_wait_ld();
+        max16m(A, lim - 32);
         max16m(B, lim - 48);  // chunk 3 stays in B for pass 2
         if (r == 0) TRACE(t, 1, tr_it);
         const float mx_half = fmaxf(mx0, mx1);
@@ -548,8 +551,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             pk[i] = pack_bf16(e.x, e.y);
           }
         };
-        auto exp16 = [&](const float* v, int k, int lim_k) {
-          uint32_t pk[8];
+        auto exp16 = [&](const float* v, int lim_k, uint32_t* pk) {
           if (!edge || lim_k >= 15) {  // (interior blocks: warp-uniform, no divergence at all)
             exp16_body(v, lim_k, pk, std::false_type{});
           } else if (lim_k < 0) {
@@ -559,7 +561,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             exp16_body(v, lim_k, pk, std::true_type{});
           }
           if (edge) __syncwarp();
-          tmem_st8(tS + 16 * k, pk);
         };
 #define RELOAD(addr, dst) tmem_ld16(addr, reinterpret_cast<uint32_t*>(dst))
         auto hand_over = [&](int slot) {  // this warp's chunk of P is in TMEM
@@ -568,20 +569,29 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           __syncwarp();
           if (lane == 0) mbar_arrive(&p_full[4 * t + slot]);
         };
-        RELOAD(tS, A);
-        exp16(B, 3, lim - 48);
+        // chunk order 3, 2, 0, 1 (slots 0..3 of the P handoff).  The store of a chunk is only
+        // waited for after the arithmetic of the next one, so tcgen05.wait::st finds it complete.
+        uint32_t pk[8];
+        RELOAD(tS + 32, A);  // (not kept from pass 1: A would be live across the O rescale)
+        exp16(B, lim - 48, pk);
+        tmem_st8(tS + 48, pk);
+        tmem_wait_ld();
+        RELOAD(tS, B);
+        exp16(A, lim - 32, pk);
         hand_over(0);
+        tmem_st8(tS + 32, pk);
         tmem_wait_ld();
-        RELOAD(tS + 16, B);
-        exp16(A, 0, lim);
+        RELOAD(tS + 16, A);
+        exp16(B, lim, pk);
         hand_over(1);
+        tmem_st8(tS, pk);
         tmem_wait_ld();
-        RELOAD(tS + 32, A);
-        exp16(B, 1, lim - 16);
+        exp16(A, lim - 16, pk);
         hand_over(2);
-        tmem_wait_ld();
-        exp16(A, 2, lim - 32);
+        tmem_st8(tS + 16, pk);
         hand_over(3);
+        };
+        if (edge_block) softmax_block(std::true_type{}); else softmax_block(std::false_type{});
         if (r == 0) TRACE(t, 3 + hf, tr_it);
         ++tr_it;
         ++cnt;
@@ -603,6 +613,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         uint32_t o[16];
         tmem_ld16(tO + c * 16, o);
         tmem_wait_ld();
+        if (c == 0 && r == 0 && hf == 0) UTRACE(t, 6, un);
         if (valid) {
           uint4 pk[2];
 #pragma unroll
@@ -622,6 +633,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           }
         }
       }
+      if (r == 0 && hf == 0) UTRACE(t, 7, un);
       if (valid && hf == 0)
         p.LSE[(int64_t)h * p.lse_head_stride + grow] =
             l > 0.f ? m_used * 0.69314718055994531f + __logf(l) : -CUDART_INF_F;
