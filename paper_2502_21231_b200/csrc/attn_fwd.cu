@@ -137,11 +137,10 @@ struct WalkerT {
       load_span();
     }
   }
-  // total blocks tile t takes part in over the whole item
+  // total blocks tile t takes part in over the whole item (counted by the host: the loop over
+  // the spans cost the MMA issuer ~1500 cycles in front of every unit's first S MMA)
   __device__ __forceinline__ int total(int t) const {
-    int n = 0;
-    for (int q = 0; q < n_spans; ++q) n += span_blocks(at0(t), rows(t), unit_span(*u, table, q));
-    return kUniform ? warp_uniform(n) : n;
+    return t ? u->item.tile_blocks[1] : u->item.tile_blocks[0];
   }
 };
 using Walker = WalkerT<false>;
@@ -410,6 +409,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           if (!has_next) break;
           cur = nxt;
         }
+        UTRACE(2 + t, 5, un);
       }
     }
   } else {
@@ -473,6 +473,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         constexpr bool edge = decltype(edge_c)::value;
         // last visible column of this row relative to this thread's first column (>= 63: all)
         const int lim = edge ? min(at0 + r + wk.sp.off, wk.sp.len - 1) - b0 - hf * 64 : 64;
+        // The same for the first and the last row of this warp (lim grows with the row): a chunk
+        // is classified for the whole warp - every row sees all of it / no row sees any of it /
+        // mixed - so that the rows of a warp never take different paths.
+        const int lim_lo = edge ? __shfl_sync(0xffffffffu, lim, 0) : 64;
+        const int lim_hi = edge ? __shfl_sync(0xffffffffu, lim, 31) : 64;
         float A[16], B[16];
         float mx0 = -CUDART_INF_F, mx1 = -CUDART_INF_F;
         auto max16 = [&](const float* v) {
@@ -485,12 +490,13 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // Pass 1: maximum over the visible columns.  It has to be exact: with an inflated
         // maximum the largest P of a row is no longer exactly 1, its bf16 rounding no longer
         // cancels against the fp32 row sum, and rows with few visible keys (the first rows of a
-        // document) lose up to 2^-9 relative in O.  Chunks without a visible column are skipped,
-        // only the row's boundary chunk pays for selects.
-        auto max16m = [&](const float* v, int lim_k) {
-          if (!edge || lim_k >= 15) {
+        // document) lose up to 2^-9 relative in O.  Chunks no row of the warp sees are skipped,
+        // chunks every row sees take the plain code, only mixed chunks pay for selects.
+        auto max16m = [&](const float* v, int k16) {
+          const int lim_k = lim - k16;
+          if (!edge || lim_lo - k16 >= 15) {
             max16(v);
-          } else if (lim_k >= 0) {
+          } else if (lim_hi - k16 >= 0) {
 #pragma unroll
             for (int c = 0; c < 16; ++c) mx0 = fmaxf(mx0, c <= lim_k ? v[c] : -CUDART_INF_F);
           }
@@ -498,13 +504,13 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tmem_ld16(tS, reinterpret_cast<uint32_t*>(A));
         tmem_ld16(tS + 16, reinterpret_cast<uint32_t*>(B));
         tmem_wait_ld();
-        max16m(A, lim);
+        max16m(A, 0);
         tmem_ld16(tS + 32, reinterpret_cast<uint32_t*>(A));
-        max16m(B, lim - 16);
+        max16m(B, 16);
         tmem_ld16(tS + 48, reinterpret_cast<uint32_t*>(B));
         tmem_wait_ld();
-        max16m(A, lim - 32);
-        max16m(B, lim - 48);  // chunk 3 stays in B for pass 2
+        max16m(A, 32);
+        max16m(B, 48);  // chunk 3 stays in B for pass 2
         if (r == 0) TRACE(t, 1, tr_it);
         const float mx_half = fmaxf(mx0, mx1);
         // exchange the half-row maxima (slots alternate with the block parity; one barrier/block)
@@ -534,10 +540,10 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (r == 0) TRACE(t, 2, tr_it);
         const float neg_m = (m_used == -CUDART_INF_F) ? 0.f : -m_used;
         const float2 nm2 = make_float2(neg_m, neg_m);
-        // P of one 16-column chunk: all columns visible (lim_k >= 15), none (lim_k < 0: zeros, no
-        // exponentials at all) or the one boundary chunk of the row, where masked columns are
-        // zeroed after the exponential.  The branches hold arithmetic only and may diverge
-        // between the rows of a warp; the tcgen05.st after them is converged again.
+        // P of one 16-column chunk, classified per warp: every row sees all of it (unmasked code),
+        // no row sees any of it (zeros, no exponentials at all), or mixed - then all rows run the
+        // masked code, which zeroes hidden columns after the exponential.  No divergence inside a
+        // warp: per-row classes made a diagonal block three times as expensive as an interior one.
         auto exp16_body = [&](const float* v, int lim_k, uint32_t* pk, auto masked) {
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
@@ -551,16 +557,16 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             pk[i] = pack_bf16(e.x, e.y);
           }
         };
-        auto exp16 = [&](const float* v, int lim_k, uint32_t* pk) {
-          if (!edge || lim_k >= 15) {  // (interior blocks: warp-uniform, no divergence at all)
+        auto exp16 = [&](const float* v, int k16, uint32_t* pk) {
+          const int lim_k = lim - k16;
+          if (!edge || lim_lo - k16 >= 15) {
             exp16_body(v, lim_k, pk, std::false_type{});
-          } else if (lim_k < 0) {
+          } else if (lim_hi - k16 < 0) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) pk[i] = 0u;
           } else {
             exp16_body(v, lim_k, pk, std::true_type{});
           }
-          if (edge) __syncwarp();
         };
 #define RELOAD(addr, dst) tmem_ld16(addr, reinterpret_cast<uint32_t*>(dst))
         auto hand_over = [&](int slot) {  // this warp's chunk of P is in TMEM
@@ -573,20 +579,20 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // waited for after the arithmetic of the next one, so tcgen05.wait::st finds it complete.
         uint32_t pk[8];
         RELOAD(tS + 32, A);  // (not kept from pass 1: A would be live across the O rescale)
-        exp16(B, lim - 48, pk);
+        exp16(B, 48, pk);
         tmem_st8(tS + 48, pk);
         tmem_wait_ld();
         RELOAD(tS, B);
-        exp16(A, lim - 32, pk);
+        exp16(A, 32, pk);
         hand_over(0);
         tmem_st8(tS + 32, pk);
         tmem_wait_ld();
         RELOAD(tS + 16, A);
-        exp16(B, lim, pk);
+        exp16(B, 0, pk);
         hand_over(1);
         tmem_st8(tS, pk);
         tmem_wait_ld();
-        exp16(A, lim - 16, pk);
+        exp16(A, 16, pk);
         hand_over(2);
         tmem_st8(tS + 16, pk);
         hand_over(3);

@@ -59,7 +59,7 @@ struct SchedRing {  // lives in shared memory (16-byte aligned)
   int32_t unit[kSchedSlots];
   uint64_t full[kSchedSlots], empty[kSchedSlots];
 };
-constexpr int kSchedRingBytes = 384;
+constexpr int kSchedRingBytes = 128 * kSchedSlots;
 static_assert(sizeof(SchedRing) <= kSchedRingBytes, "SchedRing size");
 
 // n_consumers = arrivals per slot on the empty barrier (threads calling next(), warps calling

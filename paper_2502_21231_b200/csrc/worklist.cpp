@@ -145,8 +145,9 @@ bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
           const int64_t a_last = std::min<int64_t>(at + kTile, q_len) - 1;
           for (int32_t s = span_begin; s < span_begin + it.n_spans; ++s) {
             const int64_t vis = std::min<int64_t>(out->spans[s].len, a_last + out->spans[s].off + 1);
-            if (vis > 0) cost += ceil_div(vis, kTile);
+            if (vis > 0) it.tile_blocks[t] += (int32_t)ceil_div(vis, kTile);
           }
+          cost += it.tile_blocks[t];
         }
         it.cost = cost;
         out->items.push_back(it);

@@ -37,7 +37,7 @@ struct Item {
   int32_t span_begin;  // first span in the span table
   int32_t n_spans;
   int32_t cost;        // 128x128 blocks the item visits per head
-  int32_t pad[2];
+  int32_t tile_blocks[2];  // fwd: of those, the blocks of Q tile 0 / 1 (bwd: unused)
 };
 struct Group {           // the items of one distinct range; units = n_items x heads
   int32_t item_begin;    // first item in the item table
