@@ -100,9 +100,16 @@ struct WalkerT {
   const Span* table;
   const Unit* u;
   int n_spans, s, j, nb0, nb1, at0_1, rows0, rows1;
+  int flip;  // TMEM / shared-memory slot t works on Q tile t ^ flip of the item (see tile())
   Span sp;
-  __device__ __forceinline__ int at0(int t) const { return t ? at0_1 : at0_1 - kTile; }
-  __device__ __forceinline__ int rows(int t) const { return t ? rows1 : rows0; }
+  // The upper tile of a causal pair visits one block more than the lower one.  With a fixed
+  // assignment the slot of the lower tile runs ahead by a block per unit until the K/V ring stops
+  // it, and from then on every stage is held for the trailing slot: no prefetch distance left.
+  // Alternating the assignment from unit to unit keeps the two slots within one block (a rule
+  // on the blocks given to each slot so far alternates the same way and measured no better).
+  __device__ __forceinline__ int tile(int t) const { return t ^ flip; }
+  __device__ __forceinline__ int at0(int t) const { return tile(t) ? at0_1 : at0_1 - kTile; }
+  __device__ __forceinline__ int rows(int t) const { return tile(t) ? rows1 : rows0; }
   __device__ __forceinline__ void load_span() {
     while (s < n_spans) {
       sp = unit_span(*u, table, s);
@@ -118,8 +125,9 @@ struct WalkerT {
     }
     j = 0;
   }
-  __device__ __forceinline__ void init(const Span* sp_table, const Unit& unit) {
+  __device__ __forceinline__ void init(const Span* sp_table, const Unit& unit, int flip_) {
     const Item& it = unit.item;
+    flip = flip_;
     table = sp_table;
     u = &unit;
     n_spans = it.n_spans;
@@ -130,7 +138,7 @@ struct WalkerT {
     load_span();
   }
   __device__ __forceinline__ bool done() const { return s >= n_spans; }
-  __device__ __forceinline__ bool active(int t) const { return j < (t ? nb1 : nb0); }
+  __device__ __forceinline__ bool active(int t) const { return j < (tile(t) ? nb1 : nb0); }
   __device__ __forceinline__ void next() {
     if (++j >= max(nb0, nb1)) {
       ++s;
@@ -140,7 +148,7 @@ struct WalkerT {
   // total blocks tile t takes part in over the whole item (counted by the host: the loop over
   // the spans cost the MMA issuer ~1500 cycles in front of every unit's first S MMA)
   __device__ __forceinline__ int total(int t) const {
-    return t ? u->item.tile_blocks[1] : u->item.tile_blocks[0];
+    return tile(t) ? u->item.tile_blocks[1] : u->item.tile_blocks[0];
   }
 };
 using Walker = WalkerT<false>;
@@ -259,7 +267,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           bulk_commit_group();
         }
         Walker wk;
-        wk.init(p.sv.spans, u);
+        wk.init(p.sv.spans, u, un & 1);
         if (wk.done()) continue;
         // Order of a unit's loads: K of the first block (its ring stage is released early, at
         // the S MMAs four stages back), then the two Q tiles (a tile's buffer is released at its
@@ -287,7 +295,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
               mbar_arrive_expect_tx(&q_full[t], L::kTileBytes);
               for (int half = 0; half < D / 64; ++half)
                 tma_load_3d(smem + L::kQOff + t * L::kTileBytes + half * (kTile * 128), &tmQ,
-                            &q_full[t], half * 64, h, it.row0 + t * kTile);
+                            &q_full[t], half * 64, h, it.row0 + wk.tile(t) * kTile);
             }
           }
           load_kv(1, krow);
@@ -319,7 +327,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         ++un;
         UTRACE(2 + t, 0, un);
         Walker cur;
-        cur.init(p.sv.spans, u);
+        cur.init(p.sv.spans, u, un & 1);
         if (cur.done()) continue;
         const int tot = cur.total(t);
         UTRACE(2 + t, 1, un);
@@ -437,10 +445,10 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       const Item& it = u.item;
       const int h = u.head;
       Walker wk;
-      wk.init(p.sv.spans, u);
+      wk.init(p.sv.spans, u, un & 1);
       const int at0 = wk.at0(t);
       const bool valid = r < wk.rows(t);
-      const int64_t grow = (int64_t)it.row0 + t * kTile + r;
+      const int64_t grow = (int64_t)it.row0 + wk.tile(t) * kTile + r;
       __nv_bfloat16* o_ptr = p.O + grow * p.o_row_stride + (int64_t)h * D + hf * (D / 2);
       const int tot = wk.total(t);
       if (tot == 0) {  // no key of this call is visible to any row of the tile
