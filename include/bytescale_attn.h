@@ -123,6 +123,47 @@ const int32_t* bs_plan_step_k_seq(const bs_plan_t* p, int32_t s);
 void bs_plan_destroy(bs_plan_t* p);                           /* NULL is a no-op */
 
 /* ------------------------------------------------------------------------------------------ */
+/* bs_assign: the naive HDP solution (Algorithm 1, routine at         */
+/* PAPER.md:262) with offload ratio r = 0 - the step directly upstream of bs_plan.            */
+/* ------------------------------------------------------------------------------------------ */
+/* A global batch of sequence lengths, a token capacity C per rank and d_hdp ranks become, for
+ * every rank and every round of the training step, the sequences that rank hands to bs_plan.
+ *   R1  D(s) = ceil(s / C): Eq. 3 with r = 0 and Act(s) proportional to s.
+ *       The paper's numbers at C = 8K: 1M -> 128, 16K -> 2, 768K -> 96, 312K -> 39 ranks.
+ *   R2  lines 2-6: a sequence with D(s) = 1 goes to the pack list, every other one keeps D(s).
+ *   R3  lines 7-9: one bin per pass of the while loop; the bin takes the longest remaining
+ *       sequence that still fits (ties: lowest input index) until none fits.
+ *   R4  line 10: in a round every rank runs at most one micro-batch, and the D(s) ranks of a
+ *       long sequence run it in the same round.  Long sequences are placed in input order into
+ *       the first round with D(s) free ranks, then the bins in the order they were made, each
+ *       into the first round with a free rank; a round hands out its ranks from 0 upwards
+ *       (96 ranks for a 768K sequence, the other 32 for 32 x 8K sequences).
+ * Host only, integers only; the result is unique (bit-exact contract, tests/test_assign.py). */
+typedef struct {
+  int32_t round;        /* 0 <= round < bs_assign_n_rounds */
+  int32_t rank;         /* HDP rank, 0 <= rank < d_hdp; (round, rank) is unique */
+  int32_t n_seqs;
+  const bs_seq_t* seqs; /* [n_seqs], owned by the assignment: one shard {len, cp = D, rank = j} of
+                           a long sequence, or the whole sequences {len, 1, 0} of one bin */
+  const int32_t* src;   /* [n_seqs] index of each sequence in the input batch */
+} bs_microbatch_t;
+
+typedef struct bs_assign_s bs_assign_t; /* opaque, host memory owned by the library */
+
+/* lens: host, [n].  *out receives an assignment to be released with bs_assign_destroy.
+ * Errors: INVALID_ARG (null, n < 0, len < 1, capacity < 1, d_hdp < 1, a sequence that needs
+ * more than d_hdp ranks), HOST_OOM. */
+bs_status_t bs_assign(const int32_t* lens, int32_t n, int32_t capacity, int32_t d_hdp,
+                      bs_assign_t** out);
+int32_t bs_assign_n_rounds(const bs_assign_t* a);
+int32_t bs_assign_n_seqs(const bs_assign_t* a);
+const int32_t* bs_assign_ranks_needed(const bs_assign_t* a); /* [n] D(s_i) */
+int32_t bs_assign_n_microbatches(const bs_assign_t* a);
+/* micro-batch k in (round, rank) order; NULL if k is out of range */
+const bs_microbatch_t* bs_assign_microbatch(const bs_assign_t* a, int32_t k);
+void bs_assign_destroy(bs_assign_t* a);                       /* NULL is a no-op */
+
+/* ------------------------------------------------------------------------------------------ */
 /* Device calls                                                                                */
 /* ------------------------------------------------------------------------------------------ */
 

@@ -73,6 +73,23 @@ lib.bs_plan_step.restype = _P(Step)
 lib.bs_plan_step.argtypes = [_vp, _i32]
 lib.bs_plan_destroy.restype = None
 lib.bs_plan_destroy.argtypes = [_vp]
+
+
+class Microbatch(ctypes.Structure):
+    _fields_ = [("round", _i32), ("rank", _i32), ("n_seqs", _i32), ("seqs", _P(Seq)),
+                ("src", _P(_i32))]
+
+
+lib.bs_assign.argtypes = [_P(_i32), _i32, _i32, _i32, _P(_vp)]
+for _n in ("bs_assign_n_rounds", "bs_assign_n_seqs", "bs_assign_n_microbatches"):
+    getattr(lib, _n).restype = _i32
+    getattr(lib, _n).argtypes = [_vp]
+lib.bs_assign_ranks_needed.restype = _P(_i32)
+lib.bs_assign_ranks_needed.argtypes = [_vp]
+lib.bs_assign_microbatch.restype = _P(Microbatch)
+lib.bs_assign_microbatch.argtypes = [_vp, _i32]
+lib.bs_assign_destroy.restype = None
+lib.bs_assign_destroy.argtypes = [_vp]
 lib.bs_attn_workspace_bytes.argtypes = [_P(Shape), _i32, ctypes.c_int, _P(_sz)]
 lib.bs_attn_fwd.argtypes = [_P(Shape), _vp, _vp, _vp, _P(Seg), _i32, _i32, _i32, _vp, _vp, _vp,
                             _sz, _vp, _vp]
@@ -87,7 +104,9 @@ lib.bs_launch_count_reset.restype = None
 EXPORTS = ["bs_status_string", "bs_last_error", "bs_version", "bs_plan", "bs_plan_uniform",
            "bs_plan_n_seqs", "bs_plan_q_rows", "bs_plan_cu_rows_q", "bs_plan_q_pos",
            "bs_plan_q_seq", "bs_plan_n_steps", "bs_plan_step", "bs_plan_step_k_pos",
-           "bs_plan_step_k_seq", "bs_plan_destroy", "bs_attn_workspace_bytes", "bs_attn_fwd",
+           "bs_plan_step_k_seq", "bs_plan_destroy", "bs_assign", "bs_assign_n_rounds",
+           "bs_assign_n_seqs", "bs_assign_ranks_needed", "bs_assign_n_microbatches",
+           "bs_assign_microbatch", "bs_assign_destroy", "bs_attn_workspace_bytes", "bs_attn_fwd",
            "bs_attn_bwd_prep", "bs_attn_bwd", "bs_attn_bwd_finish", "bs_lse_merge",
            "bs_launch_count", "bs_launch_count_reset"]
 
@@ -130,6 +149,27 @@ def plan(seqs):
         return _plan_to_dict(h)
     finally:
         lib.bs_plan_destroy(h)
+
+
+def assign(lens, capacity, d_hdp):
+    """bs_assign: global batch of lengths -> {"d": [D(s_i)], "n_rounds": R, "microbatches":
+    [(round, rank, [(len, cp, cp_rank, input index), ...]), ...]} in (round, rank) order."""
+    lens = [int(x) for x in lens]
+    arr = (_i32 * max(len(lens), 1))(*lens)
+    h = _vp()
+    _check(lib.bs_assign(arr, len(lens), int(capacity), int(d_hdp), ctypes.byref(h)), "bs_assign")
+    try:
+        n = lib.bs_assign_n_seqs(h)
+        d = lib.bs_assign_ranks_needed(h)
+        mbs = []
+        for k in range(lib.bs_assign_n_microbatches(h)):
+            m = lib.bs_assign_microbatch(h, k).contents
+            mbs.append((m.round, m.rank, [(m.seqs[i].len, m.seqs[i].cp, m.seqs[i].rank, m.src[i])
+                                          for i in range(m.n_seqs)]))
+        return {"d": [d[i] for i in range(n)], "n_rounds": lib.bs_assign_n_rounds(h),
+                "microbatches": mbs}
+    finally:
+        lib.bs_assign_destroy(h)
 
 
 def plan_uniform(lens, cp, rank, min_shard_len):
