@@ -28,6 +28,8 @@ METRIC = "varlen causal attn fwd+bwd TFLOP/s (unmasked)"
 WORKLOAD = "cfg2_7B_packed_32k"
 ORACLE_SAMPLE_HEADS = 1  # heads of cfg2 per step of the reference arm (MHA heads are independent)
 CPU_BASELINE_HEADS = 5    # heads the cpu_baseline leg of the default run times (~12 s)
+# bs_assign replay: global batch, rank capacity and number of HDP ranks
+HDP_CAPACITY, HDP_RANKS, HDP_N_SHORT, HDP_LONG_MULTIPLES = 8192, 16, 96, (8, 4, 2, 2)
 
 
 def peaks():
@@ -278,6 +280,14 @@ def run_ours(args, rank, world, local_rank):
         nb = lambda t: t.numel() * t.element_size()  # noqa: E731
         merge = bench_merge(B, torch, pk)
         ring = bench_ring_steps(B, torch, workloads, pk)
+        # naive HDP assignment (bs_assign) of a synthetic global batch,
+        # every rank's micro-batches replayed on this GPU
+        from paper_2502_21231_b200 import replay as RP
+        hdp_lens = RP.global_batch(w.seed, HDP_N_SHORT, HDP_CAPACITY, HDP_LONG_MULTIPLES)
+        hdp = RP.replay(hdp_lens, HDP_CAPACITY, HDP_RANKS, Hq, Hkv, D, seed=w.seed)
+        hdp["workload"] = (f"{HDP_N_SHORT} log-normal short sequences + long ones of "
+                           f"{list(HDP_LONG_MULTIPLES)} x capacity, capacity {HDP_CAPACITY} tokens, "
+                           f"d_hdp {HDP_RANKS}, {Hq} heads, D {D}")
         dt, fl, thr = oracle_sample_run(w, CPU_BASELINE_HEADS)
         bwd_tflops = 10.0 * D * Hq * pairs / (t_bwd * 1e-3) / 1e12
         out = {
@@ -300,6 +310,7 @@ def run_ours(args, rank, world, local_rank):
                          "traffic": ncu_traffic("attn_bwd_kernel")},
             "merge": merge,
             "ring_steps_cfg3_4_5": ring,
+            "hdp_naive_replay": hdp,
             "cpu_baseline": {"value": fl / dt / 1e12, "unit": "TFLOP/s", "cores": thr, "kind": "oracle",
                              "sample": f"{CPU_BASELINE_HEADS} of {Hq} heads of {WORKLOAD}, all "
                                        f"{rows} tokens, fwd+bwd, fp64, {dt:.1f} s"},

@@ -1,0 +1,105 @@
+"""Replay of a `bs_assign` result on one GPU: every micro-batch of every HDP rank is planned
+(`bs_plan`) and run through the attention hot path (forward of every ring step + LSE merge, then
+prep / backward of every ring step / finish), one after the other, timed with CUDA events.  The
+per-rank totals give the picture of PAPER.md:405 (naive HDP: "significant time variance across
+ranks ... min=60s, max=279s, std=68s") for this library's kernels on a synthetic global batch.
+
+What is replayed is each rank's own compute; the ring exchange of K/V chunks between ranks is
+outside the north_star, so the K/V buffer of a step holds seeded random rows of the right count.
+Timing only: parity of the sharded path against the oracle is the job of tests/."""
+import math
+
+import torch
+
+from . import binding as B
+
+
+def global_batch(seed, n_short, capacity, long_multiples):
+    """Synthetic global batch (stand-in for the long-tailed length histograms of PAPER.md:85,107,
+    which are not available here): `n_short` log-normal lengths clipped to [64, capacity], and one
+    sequence of m * capacity tokens for every m in `long_multiples`; input order shuffled."""
+    g = torch.Generator().manual_seed(seed)
+    mu, sigma = math.log(capacity / 8.0), 1.0
+    short = torch.exp(mu + sigma * torch.randn(n_short, generator=g)).clamp(64, capacity).long()
+    lens = [int(x) for x in short] + [int(m * capacity) for m in long_multiples]
+    perm = torch.randperm(len(lens), generator=g)
+    return [lens[int(i)] for i in perm]
+
+
+def _run_microbatch(seqs, Hq, Hkv, D, gen):
+    """One micro-batch on this GPU; returns (milliseconds, visible pairs per head)."""
+    pl = B.plan([(s[0], s[1], s[2]) for s in seqs])
+    rows, n_steps = pl["q_rows"], pl["n_steps"]
+    if rows == 0:
+        return 0.0, 0
+    dev = "cuda"
+    Q = torch.randn(rows, Hq, D, device=dev, generator=gen).bfloat16()
+    dO = torch.randn(rows, Hq, D, device=dev, generator=gen).bfloat16()
+    Ks, Vs, shapes, ws_f, ws_b = [], [], [], [], []
+    for st in pl["steps"]:
+        kv = st["kv_rows"]
+        Ks.append(torch.randn(kv, Hkv, D, device=dev, generator=gen).bfloat16())
+        Vs.append(torch.randn(kv, Hkv, D, device=dev, generator=gen).bfloat16())
+        sh = B.make_shape(Hq, Hkv, D, rows, kv)
+        shapes.append(sh)
+        ws_f.append(torch.empty(B.attn_workspace_bytes(sh, len(st["segs"]), False), dtype=torch.uint8,
+                                device=dev))
+        ws_b.append(torch.empty(B.attn_workspace_bytes(sh, len(st["segs"]), True), dtype=torch.uint8,
+                                device=dev))
+    parts_O = [torch.empty_like(Q) for _ in range(n_steps)]
+    parts_L = [torch.empty((Hq, rows), dtype=torch.float32, device=dev) for _ in range(n_steps)]
+    O = torch.empty_like(Q) if n_steps > 1 else parts_O[0]
+    LSE = torch.empty_like(parts_L[0]) if n_steps > 1 else parts_L[0]
+    delta = torch.empty_like(parts_L[0])
+    acc = torch.empty((rows, Hq, D), dtype=torch.float32, device=dev)
+    dQ = torch.empty_like(Q)
+    dKs, dVs = [torch.empty_like(k) for k in Ks], [torch.empty_like(v) for v in Vs]
+
+    def step():
+        for s, st in enumerate(pl["steps"]):
+            B.attn_fwd(shapes[s], Q, Ks[s], Vs[s], st["segs"], (0, rows), parts_O[s], parts_L[s],
+                       ws_f[s], acc if s == 0 else None)
+        if n_steps > 1:
+            B.lse_merge(parts_O, parts_L, shapes[0], (0, rows), O, LSE)
+        B.attn_bwd_prep(shapes[0], O, dO, delta, None)
+        for s, st in enumerate(pl["steps"]):
+            B.attn_bwd(shapes[s], Q, Ks[s], Vs[s], dO, LSE, delta, st["segs"], acc, dKs[s], dVs[s],
+                       ws_b[s])
+        B.attn_bwd_finish(shapes[0], acc, dQ)
+
+    step()  # warm-up (first touch of the buffers)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    step()
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b), sum(st["visible_pairs"] for st in pl["steps"])
+
+
+def replay(lens, capacity, d_hdp, n_q_heads, n_kv_heads, head_dim, seed=0):
+    """Runs every micro-batch of bs_assign(lens, capacity, d_hdp) and returns the per-rank picture:
+    {"n_rounds", "rank_ms": [d_hdp], "min_ms", "max_ms", "mean_ms", "std_ms", "max_over_min",
+     "idle_frac": share of rank-time spent waiting for the slowest rank, "tflops": unmasked
+     fwd+bwd rate over the summed compute time}."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("replay needs a CUDA device (there is no CPU path)")
+    a = B.assign(lens, capacity, d_hdp)
+    gen = torch.Generator(device="cuda").manual_seed(seed)
+    rank_ms = [0.0] * d_hdp
+    pairs = 0
+    for rnd, rank, seqs in a["microbatches"]:
+        ms, p = _run_microbatch(seqs, n_q_heads, n_kv_heads, head_dim, gen)
+        rank_ms[rank] += ms
+        pairs += p
+    t = torch.tensor(rank_ms, dtype=torch.float64)
+    busy = float(t.sum())
+    return {"n_rounds": a["n_rounds"], "n_microbatches": len(a["microbatches"]),
+            "ranks_needed_max": max(a["d"]) if a["d"] else 0,
+            "rank_ms": [round(x, 3) for x in rank_ms],
+            "min_ms": round(float(t.min()), 3), "max_ms": round(float(t.max()), 3),
+            "mean_ms": round(float(t.mean()), 3), "std_ms": round(float(t.std(unbiased=False)), 3),
+            "max_over_min": round(float(t.max() / t.min()), 2) if float(t.min()) > 0 else None,
+            "idle_frac": round(1.0 - busy / (float(t.max()) * d_hdp), 3) if busy > 0 else None,
+            "tflops": round(14.0 * head_dim * n_q_heads * pairs / (busy * 1e-3) / 1e12, 1)
+            if busy > 0 else None}

@@ -1,0 +1,23 @@
+"""-m gpu: the bs_assign replay (paper_2502_21231_b200/replay.py) runs every micro-batch of a
+small global batch through the C-ABI calls and reports a consistent per-rank picture."""
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2502_21231_b200 import binding as B  # noqa: E402
+from paper_2502_21231_b200 import replay as RP  # noqa: E402
+
+
+def test_replay_of_a_small_global_batch():
+    cap, d_hdp = 512, 4
+    lens = RP.global_batch(3, 12, cap, (3, 2))
+    assert sorted(lens)[-2:] == [2 * cap, 3 * cap] and len(lens) == 14
+    a = B.assign(lens, cap, d_hdp)
+    r = RP.replay(lens, cap, d_hdp, 4, 2, 64, seed=3)
+    assert r["n_rounds"] == a["n_rounds"] and r["n_microbatches"] == len(a["microbatches"])
+    assert len(r["rank_ms"]) == d_hdp and r["ranks_needed_max"] == 3
+    busy = {rank for _, rank, _ in a["microbatches"]}
+    for rank, ms in enumerate(r["rank_ms"]):
+        assert (ms > 0) == (rank in busy)
+    assert r["min_ms"] <= r["mean_ms"] <= r["max_ms"] and 0.0 <= r["idle_frac"] < 1.0
+    assert r["tflops"] > 0
