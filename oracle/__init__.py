@@ -7,3 +7,5 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 from .attn import (attn_bwd, attn_fwd, bf16_to_f64, build, merge, rows_from_plan,  # noqa: F401
                    threads)
 from .plan import plan as oracle_plan  # noqa: F401
+from .assign import assign as oracle_assign  # noqa: F401
+from .balance import balance as oracle_balance  # noqa: F401

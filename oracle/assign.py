@@ -28,9 +28,9 @@ def ranks_needed(s, capacity):
     return -(-s // capacity)
 
 
-def assign(lens, capacity, d_hdp):
-    """Returns {"d": [D(s_i)], "n_rounds": R, "microbatches": [(round, rank, [(len, cp, cp_rank,
-    input index), ...]), ...]} with the micro-batches sorted by (round, rank)."""
+def groups(lens, capacity, d_hdp):
+    """Lines 1-9 of Algorithm 1: (d, long_list, bins) - D(s_i) of every sequence, the indices of
+    the long sequences in input order, the bins (lists of indices) in the order they are made."""
     if capacity < 1 or d_hdp < 1 or any(s < 1 for s in lens):
         raise ValueError("bad argument")
     # lines 1-6
@@ -52,6 +52,13 @@ def assign(lens, capacity, d_hdp):
             pack_list.remove(best)
             room -= lens[best]
         bins.append(subset)
+    return d, long_list, bins
+
+
+def assign(lens, capacity, d_hdp):
+    """Returns {"d": [D(s_i)], "n_rounds": R, "microbatches": [(round, rank, [(len, cp, cp_rank,
+    input index), ...]), ...]} with the micro-batches sorted by (round, rank)."""
+    d, long_list, bins = groups(lens, capacity, d_hdp)
     # line 10 (R4)
     free = []          # free ranks of each round
     out = []
