@@ -164,6 +164,52 @@ const bs_microbatch_t* bs_assign_microbatch(const bs_assign_t* a, int32_t k);
 void bs_assign_destroy(bs_assign_t* a);                       /* NULL is a no-op */
 
 /* ------------------------------------------------------------------------------------------ */
+/* bs_balance: the balance strategy for HDP (Algorithm 2, sections     */
+/* 6.3-6.4) in its DP-Balance form; it takes the place of line 10 of Algorithm 1.              */
+/* ------------------------------------------------------------------------------------------ */
+/* Schedules the groups of Algorithm 1 lines 1-9 (a long sequence on D(s) ranks, or a bin of
+ * short ones on one rank) so that all ranks finish at about the same time; ranks may run
+ * different numbers of micro-batches.
+ *   B1  cost[3] = {a2, a1, a0}: T(s) = a2 s^2 + a1 s + a0 (Eq. 3), non-negative
+ *       integers in the caller's time unit.  A long sequence costs each of its D ranks
+ *       floor(T(s) / D), a bin the sum of T over its sequences.
+ *   B2  line 4: groups sorted by the time they cost one rank, descending (ties: more ranks
+ *       first, then the order Algorithm 1 made them).
+ *   B3  line 5: group g of the sorted list goes to bucket floor(n_buckets * work before g /
+ *       total work), at most n_buckets - 1; work = time x ranks.
+ *   B4  lines 7-9: targets = ranks more than delta behind the slowest rank; if there is none,
+ *       a new time step begins and every rank is a target.
+ *   B5  lines 10-17: the next group of the first bucket goes to the D targets with the smallest
+ *       exec_times (ties: lowest rank; if fewer than D ranks are targets the least loaded others
+ *       fill up); they start together at the largest of their exec_times.  CP rank j is the j-th
+ *       chosen rank in ascending order.
+ *   B6  lines 18-20: an empty bucket is removed.
+ * Under B4/B5 the targets are a prefix of the ranks ordered by exec_time, so the result does not
+ * depend on n_buckets and delta (they matter for PP-Balance, which is out of scope); both are
+ * validated and otherwise unused.  Host only, integers only, unique result. */
+typedef struct {
+  int32_t rank;         /* HDP rank */
+  int32_t n_seqs;
+  int64_t start, end;   /* in the unit of cost[]; a rank's micro-batches do not overlap */
+  const bs_seq_t* seqs; /* [n_seqs] as in bs_microbatch_t */
+  const int32_t* src;   /* [n_seqs] index of each sequence in the input batch */
+} bs_timed_microbatch_t;
+
+typedef struct bs_balance_s bs_balance_t; /* opaque, host memory owned by the library */
+
+/* Errors: INVALID_ARG (as bs_assign; negative cost or delta, n_buckets < 1, a sequence cost
+ * >= 2^53 or a total >= 2^62), HOST_OOM. */
+bs_status_t bs_balance(const int32_t* lens, int32_t n, int32_t capacity, int32_t d_hdp,
+                       const int64_t* cost, int32_t n_buckets, int64_t delta, bs_balance_t** out);
+int32_t bs_balance_n_ranks(const bs_balance_t* b);
+const int64_t* bs_balance_exec_times(const bs_balance_t* b); /* [d_hdp] finish time of each rank */
+int64_t bs_balance_makespan(const bs_balance_t* b);
+int32_t bs_balance_n_microbatches(const bs_balance_t* b);
+/* micro-batch k in (rank, start) order; NULL if k is out of range */
+const bs_timed_microbatch_t* bs_balance_microbatch(const bs_balance_t* b, int32_t k);
+void bs_balance_destroy(bs_balance_t* b);                     /* NULL is a no-op */
+
+/* ------------------------------------------------------------------------------------------ */
 /* Device calls                                                                                */
 /* ------------------------------------------------------------------------------------------ */
 

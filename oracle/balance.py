@@ -13,7 +13,8 @@ B2  line 4 "sort B by sequence length in descending order": the groups are sorte
     they cost one rank, descending (ties: more ranks first, then the order Algorithm 1 made them).
 B3  line 5 "divide B into buckets such that each bucket has an approximately equal sum of FLOPs":
     with n_buckets given, group g of the sorted list goes to bucket
-    floor(n_buckets * (work of the groups before g) / (total work)), work = time x ranks.
+    floor(n_buckets * (work of the groups before g) / (total work)), work = time x ranks (a
+    group of zero work behind all the work stays in the last bucket).
 B4  lines 7-9: max_time = max(exec_times); target ranks = {i : max_time - exec_times[i] > delta}.
     When no rank lags by more than delta (first of all at the start, all times 0) a new time
     step begins and every rank is a target.
@@ -60,7 +61,7 @@ def balance(lens, capacity, d_hdp, cost, n_buckets=4, delta=0):
     buckets = [[] for _ in range(n_buckets)]
     before = 0
     for g in order:
-        b = (n_buckets * before) // total if total > 0 else 0
+        b = min(n_buckets - 1, (n_buckets * before) // total) if total > 0 else 0
         buckets[b].append(g)
         before += items[g]["time"] * items[g]["ranks"]
     buckets = [b for b in buckets if b]

@@ -90,6 +90,25 @@ lib.bs_assign_microbatch.restype = _P(Microbatch)
 lib.bs_assign_microbatch.argtypes = [_vp, _i32]
 lib.bs_assign_destroy.restype = None
 lib.bs_assign_destroy.argtypes = [_vp]
+
+
+class TimedMicrobatch(ctypes.Structure):
+    _fields_ = [("rank", _i32), ("n_seqs", _i32), ("start", _i64), ("end", _i64),
+                ("seqs", _P(Seq)), ("src", _P(_i32))]
+
+
+lib.bs_balance.argtypes = [_P(_i32), _i32, _i32, _i32, _P(_i64), _i32, _i64, _P(_vp)]
+for _n in ("bs_balance_n_ranks", "bs_balance_n_microbatches"):
+    getattr(lib, _n).restype = _i32
+    getattr(lib, _n).argtypes = [_vp]
+lib.bs_balance_exec_times.restype = _P(_i64)
+lib.bs_balance_exec_times.argtypes = [_vp]
+lib.bs_balance_makespan.restype = _i64
+lib.bs_balance_makespan.argtypes = [_vp]
+lib.bs_balance_microbatch.restype = _P(TimedMicrobatch)
+lib.bs_balance_microbatch.argtypes = [_vp, _i32]
+lib.bs_balance_destroy.restype = None
+lib.bs_balance_destroy.argtypes = [_vp]
 lib.bs_attn_workspace_bytes.argtypes = [_P(Shape), _i32, ctypes.c_int, _P(_sz)]
 lib.bs_attn_fwd.argtypes = [_P(Shape), _vp, _vp, _vp, _P(Seg), _i32, _i32, _i32, _vp, _vp, _vp,
                             _sz, _vp, _vp]
@@ -106,7 +125,9 @@ EXPORTS = ["bs_status_string", "bs_last_error", "bs_version", "bs_plan", "bs_pla
            "bs_plan_q_seq", "bs_plan_n_steps", "bs_plan_step", "bs_plan_step_k_pos",
            "bs_plan_step_k_seq", "bs_plan_destroy", "bs_assign", "bs_assign_n_rounds",
            "bs_assign_n_seqs", "bs_assign_ranks_needed", "bs_assign_n_microbatches",
-           "bs_assign_microbatch", "bs_assign_destroy", "bs_attn_workspace_bytes", "bs_attn_fwd",
+           "bs_assign_microbatch", "bs_assign_destroy", "bs_balance", "bs_balance_n_ranks",
+           "bs_balance_exec_times", "bs_balance_makespan", "bs_balance_n_microbatches",
+           "bs_balance_microbatch", "bs_balance_destroy", "bs_attn_workspace_bytes", "bs_attn_fwd",
            "bs_attn_bwd_prep", "bs_attn_bwd", "bs_attn_bwd_finish", "bs_lse_merge",
            "bs_launch_count", "bs_launch_count_reset"]
 
@@ -170,6 +191,28 @@ def assign(lens, capacity, d_hdp):
                 "microbatches": mbs}
     finally:
         lib.bs_assign_destroy(h)
+
+
+def balance(lens, capacity, d_hdp, cost, n_buckets=4, delta=0):
+    """bs_balance: {"exec_times": [d_hdp], "makespan", "microbatches": [(rank, start, end,
+    [(len, cp, cp_rank, input index), ...]), ...]} in (rank, start) order."""
+    lens = [int(x) for x in lens]
+    arr = (_i32 * max(len(lens), 1))(*lens)
+    c = (_i64 * 3)(*[int(x) for x in cost])
+    h = _vp()
+    _check(lib.bs_balance(arr, len(lens), int(capacity), int(d_hdp), c, int(n_buckets), int(delta),
+                          ctypes.byref(h)), "bs_balance")
+    try:
+        t = lib.bs_balance_exec_times(h)
+        mbs = []
+        for k in range(lib.bs_balance_n_microbatches(h)):
+            m = lib.bs_balance_microbatch(h, k).contents
+            mbs.append((m.rank, m.start, m.end,
+                        [(m.seqs[i].len, m.seqs[i].cp, m.seqs[i].rank, m.src[i]) for i in range(m.n_seqs)]))
+        return {"exec_times": [t[i] for i in range(lib.bs_balance_n_ranks(h))],
+                "makespan": lib.bs_balance_makespan(h), "microbatches": mbs}
+    finally:
+        lib.bs_balance_destroy(h)
 
 
 def plan_uniform(lens, cp, rank, min_shard_len):

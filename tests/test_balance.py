@@ -13,8 +13,6 @@ import oracle.balance as OB
 
 def lib_balance(lens, capacity, d_hdp, cost, n_buckets=4, delta=0):
     from paper_2502_21231_b200 import binding as B
-    if not hasattr(B, "balance"):
-        pytest.skip("bs_balance is not built yet (the oracle and its pins come first)")
     return B.balance(lens, capacity, d_hdp, cost, n_buckets, delta)
 
 
