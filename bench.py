@@ -29,7 +29,7 @@ WORKLOAD = "cfg2_7B_packed_32k"
 ORACLE_SAMPLE_HEADS = 1  # heads of cfg2 per step of the reference arm (MHA heads are independent)
 CPU_BASELINE_HEADS = 5    # heads the cpu_baseline leg of the default run times (~12 s)
 # bs_assign replay: global batch, rank capacity and number of HDP ranks
-HDP_CAPACITY, HDP_RANKS, HDP_N_SHORT, HDP_LONG_MULTIPLES = 8192, 16, 96, (8, 4, 2, 2)
+HDP_CAPACITY, HDP_RANKS, HDP_N_SHORT, HDP_LONG_MULTIPLES = 8192, 16, 384, (8, 4, 2, 2)
 
 
 def peaks():
@@ -285,6 +285,7 @@ def run_ours(args, rank, world, local_rank):
         from paper_2502_21231_b200 import replay as RP
         hdp_lens = RP.global_batch(w.seed, HDP_N_SHORT, HDP_CAPACITY, HDP_LONG_MULTIPLES)
         hdp = RP.replay(hdp_lens, HDP_CAPACITY, HDP_RANKS, Hq, Hkv, D, seed=w.seed)
+        hdp_bal = RP.replay_balanced(hdp_lens, HDP_CAPACITY, HDP_RANKS, Hq, Hkv, D, seed=w.seed)
         hdp["workload"] = (f"{HDP_N_SHORT} log-normal short sequences + long ones of "
                            f"{list(HDP_LONG_MULTIPLES)} x capacity, capacity {HDP_CAPACITY} tokens, "
                            f"d_hdp {HDP_RANKS}, {Hq} heads, D {D}")
@@ -311,6 +312,7 @@ def run_ours(args, rank, world, local_rank):
             "merge": merge,
             "ring_steps_cfg3_4_5": ring,
             "hdp_naive_replay": hdp,
+            "hdp_balance_replay": hdp_bal,
             "cpu_baseline": {"value": fl / dt / 1e12, "unit": "TFLOP/s", "cores": thr, "kind": "oracle",
                              "sample": f"{CPU_BASELINE_HEADS} of {Hq} heads of {WORKLOAD}, all "
                                        f"{rows} tokens, fwd+bwd, fp64, {dt:.1f} s"},

@@ -103,3 +103,79 @@ def replay(lens, capacity, d_hdp, n_q_heads, n_kv_heads, head_dim, seed=0):
             "idle_frac": round(1.0 - busy / (float(t.max()) * d_hdp), 3) if busy > 0 else None,
             "tflops": round(14.0 * head_dim * n_q_heads * pairs / (busy * 1e-3) / 1e12, 1)
             if busy > 0 else None}
+
+
+def fit_cost_model(n_q_heads, n_kv_heads, head_dim, lengths=(512, 1024, 2048, 4096, 8192), seed=0):
+    """T(s) = a2 s^2 + a1 s + a0 (Eq. 3) fitted by least squares to the measured
+    fwd+bwd time of one whole sequence of s tokens on this GPU.  Returns non-negative integer
+    coefficients in femtoseconds (the unit bs_balance schedules in) and the measured points."""
+    gen = torch.Generator(device="cuda").manual_seed(seed)
+    pts = []
+    for s in lengths:
+        ms = min(_run_microbatch([(s, 1, 0, 0)], n_q_heads, n_kv_heads, head_dim, gen)[0]
+                 for _ in range(3))
+        pts.append((s, ms))
+    x = torch.tensor([[float(s) * s, float(s), 1.0] for s, _ in pts], dtype=torch.float64)
+    y = torch.tensor([ms * 1e12 for _, ms in pts], dtype=torch.float64)   # ms -> fs
+    coef = torch.linalg.lstsq(x, y.unsqueeze(1)).solution.squeeze(1)
+    return [max(0, int(round(float(c)))) for c in coef], pts
+
+
+def _timeline(microbatches, d_hdp, duration):
+    """Per-rank finish times when the micro-batches run in schedule order and the ranks of a long
+    sequence start together.  microbatches: [(rank, start, end, seqs)], duration(k) in ms."""
+    order = sorted(range(len(microbatches)), key=lambda k: (microbatches[k][1], microbatches[k][0]))
+    now = [0.0] * d_hdp
+    busy = [0.0] * d_hdp
+    gangs = {}
+    for k in order:
+        rank, _, _, seqs = microbatches[k]
+        if seqs[0][1] > 1:
+            gangs.setdefault(seqs[0][3], []).append(k)
+    done = set()
+    for k in order:
+        if k in done:
+            continue
+        rank, _, _, seqs = microbatches[k]
+        members = gangs[seqs[0][3]] if seqs[0][1] > 1 else [k]
+        ranks = [microbatches[m][0] for m in members]
+        start = max(now[r] for r in ranks)
+        end = start + max(duration(m) for m in members)
+        for m, r in zip(members, ranks):
+            now[r] = end
+            busy[r] += duration(m)
+            done.add(m)
+    return now, busy
+
+
+def replay_balanced(lens, capacity, d_hdp, n_q_heads, n_kv_heads, head_dim, seed=0):
+    """Algorithm 2 (bs_balance) on the cost model fitted to this GPU, next to Algorithm 1's own
+    line 10 (bs_assign): makespans under the model, and the balanced schedule replayed on the GPU
+    (every micro-batch run and timed, the ranks of a long sequence starting together)."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("replay needs a CUDA device (there is no CPU path)")
+    cost, pts = fit_cost_model(n_q_heads, n_kv_heads, head_dim, seed=seed)
+    bal = B.balance(lens, capacity, d_hdp, cost)
+    naive = B.assign(lens, capacity, d_hdp)
+
+    def model_ms(seqs):
+        t = sum(cost[0] * s[0] * s[0] + cost[1] * s[0] + cost[2] for s in seqs)
+        return (t // seqs[0][1] if seqs[0][1] > 1 else t) * 1e-12
+    naive_t = [0.0] * d_hdp
+    for _, rank, seqs in naive["microbatches"]:
+        naive_t[rank] += model_ms(seqs)
+    gen = torch.Generator(device="cuda").manual_seed(seed)
+    measured = [_run_microbatch(seqs, n_q_heads, n_kv_heads, head_dim, gen)[0]
+                for _, _, _, seqs in bal["microbatches"]]
+    finish, busy = _timeline(bal["microbatches"], d_hdp, lambda k: measured[k])
+    t = torch.tensor(finish, dtype=torch.float64)
+    return {"cost_fs": cost, "fit_points_ms": [(s, round(ms, 4)) for s, ms in pts],
+            "model": {"naive_makespan_ms": round(max(naive_t), 3),
+                      "balance_makespan_ms": round(bal["makespan"] * 1e-12, 3),
+                      "speedup": round(max(naive_t) / (bal["makespan"] * 1e-12), 3)},
+            "measured": {"rank_finish_ms": [round(x, 3) for x in finish],
+                         "min_ms": round(float(t.min()), 3), "max_ms": round(float(t.max()), 3),
+                         "std_ms": round(float(t.std(unbiased=False)), 3),
+                         "max_over_min": round(float(t.max() / t.min()), 2) if float(t.min()) > 0 else None,
+                         "idle_frac": round(1.0 - sum(busy) / (float(t.max()) * d_hdp), 3)},
+            "n_microbatches": len(bal["microbatches"])}

@@ -21,3 +21,17 @@ def test_replay_of_a_small_global_batch():
         assert (ms > 0) == (rank in busy)
     assert r["min_ms"] <= r["mean_ms"] <= r["max_ms"] and 0.0 <= r["idle_frac"] < 1.0
     assert r["tflops"] > 0
+
+
+def test_balanced_replay_of_a_small_global_batch():
+    cap, d_hdp = 512, 4
+    lens = RP.global_batch(3, 24, cap, (3, 2))
+    r = RP.replay_balanced(lens, cap, d_hdp, 4, 2, 64, seed=3)
+    assert len(r["cost_fs"]) == 3 and all(c >= 0 for c in r["cost_fs"]) and sum(r["cost_fs"]) > 0
+    bal = B.balance(lens, cap, d_hdp, r["cost_fs"])
+    assert r["n_microbatches"] == len(bal["microbatches"])
+    assert abs(r["model"]["balance_makespan_ms"] - bal["makespan"] * 1e-12) < 1e-3
+    assert r["model"]["balance_makespan_ms"] <= r["model"]["naive_makespan_ms"] + 1e-9
+    m = r["measured"]
+    assert len(m["rank_finish_ms"]) == d_hdp and m["min_ms"] <= m["max_ms"]
+    assert 0.0 <= m["idle_frac"] < 1.0
