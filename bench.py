@@ -279,6 +279,7 @@ def run_ours(args, rank, world, local_rank):
         pk = peaks()
         nb = lambda t: t.numel() * t.element_size()  # noqa: E731
         merge = bench_merge(B, torch, pk)
+        xent = bench_softmax_xent(B, torch, pk)
         ring = bench_ring_steps(B, torch, workloads, pk)
         # naive HDP assignment (bs_assign) of a synthetic global batch,
         # every rank's micro-batches replayed on this GPU
@@ -310,6 +311,7 @@ def run_ours(args, rank, world, local_rank):
                          "peak": pk["tflops"], "unit": "TFLOP/s", "frac": bwd_tflops / pk["tflops"],
                          "traffic": ncu_traffic("attn_bwd_kernel")},
             "merge": merge,
+            "softmax_xent": xent,
             "ring_steps_cfg3_4_5": ring,
             "hdp_naive_replay": hdp,
             "hdp_balance_replay": hdp_bal,
@@ -350,6 +352,34 @@ def bench_merge(B, torch, pk):
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s",
                          "frac": gbs / pk["hbm"], "frac_of_nominal_8000": gbs / 8000.0,
                          "traffic": ncu_traffic("lse_merge_kernel")}}
+
+
+def bench_softmax_xent(B, torch, pk):
+    """bs_softmax_xent: 32768 tokens x 16384 logits (a 128K
+    vocabulary under TP = 8), bf16 in / bf16 gradients out, 2.1 GB per call (> L2)."""
+    T, V = 32768, 16384
+    x = (torch.randn(T, V, device="cuda") * 3).bfloat16()
+    y = torch.randint(0, V, (T,), device="cuda", dtype=torch.int32)
+    loss, d = torch.empty(T, device="cuda"), torch.empty_like(x)
+    for _ in range(3):
+        B.softmax_xent(x, y, 1.0 / T, loss, d)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    it = 10
+    e0.record()
+    for _ in range(it):
+        B.softmax_xent(x, y, 1.0 / T, loss, d)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / it
+    nbytes = T * V * 4 + T * 8
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    del x, d
+    torch.cuda.empty_cache()
+    return {"workload": f"{T} tokens x {V} logits (128K vocabulary / TP 8), bf16", "ms": ms,
+            "bytes": nbytes,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s",
+                         "frac": gbs / pk["hbm"], "frac_of_nominal_8000": gbs / 8000.0,
+                         "traffic": ncu_traffic("softmax_xent")}}
 
 
 def bench_ring_steps(B, torch, workloads, pk):

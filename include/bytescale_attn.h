@@ -281,6 +281,22 @@ bs_status_t bs_lse_merge(int32_t n_parts, const void* const* O_parts,
                          int32_t row_begin, int32_t row_end, void* O_out, float* LSE_out,
                          void* stream);
 
+/* ------------------------------------------------------------------------------------------ */
+/* Fused softmax cross-entropy                              */
+/* ------------------------------------------------------------------------------------------ */
+/* One kernel, bf16 in, fp32 online softmax inside, one read of the logits and one write of the
+ * gradients.  For token i with label y_i >= 0:
+ *     loss[i]       = log(sum_j exp(x_ij)) - x_i[y_i]
+ *     dlogits[i][j] = grad_scale * (softmax(x_i)[j] - (j == y_i))
+ * and loss[i] = 0, dlogits[i][:] = 0 for y_i < 0 (ignored token).
+ * logits, dlogits: device, bf16, [n_tokens][row_stride] with the first `vocab` columns used
+ * (row_stride in elements, >= vocab, a multiple of 8; both 16-byte aligned; they may not
+ * alias).  labels: device, int32 [n_tokens], < vocab.  loss: device, fp32 [n_tokens].
+ * Errors: INVALID_ARG (sizes, stride, alignment, null pointers), CUDA.  Asynchronous on stream. */
+bs_status_t bs_softmax_xent(const void* logits, const int32_t* labels, int32_t n_tokens,
+                            int32_t vocab, int64_t row_stride, float grad_scale, float* loss,
+                            void* dlogits, void* stream);
+
 /* Number of kernels this library has launched on the calling thread since the last reset
  * (bench.py's "gpu_launches"). */
 int64_t bs_launch_count(void);

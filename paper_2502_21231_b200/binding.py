@@ -117,6 +117,7 @@ lib.bs_attn_bwd.argtypes = [_P(Shape), _vp, _vp, _vp, _vp, _vp, _vp, _P(Seg), _i
                             _vp, _sz, _vp]
 lib.bs_attn_bwd_finish.argtypes = [_P(Shape), _vp, _vp, _vp]
 lib.bs_lse_merge.argtypes = [_i32, _P(_vp), _P(_vp), _P(Shape), _i32, _i32, _vp, _vp, _vp]
+lib.bs_softmax_xent.argtypes = [_vp, _vp, _i32, _i32, _i64, ctypes.c_float, _vp, _vp, _vp]
 lib.bs_launch_count.restype = _i64
 lib.bs_launch_count_reset.restype = None
 
@@ -128,7 +129,7 @@ EXPORTS = ["bs_status_string", "bs_last_error", "bs_version", "bs_plan", "bs_pla
            "bs_assign_microbatch", "bs_assign_destroy", "bs_balance", "bs_balance_n_ranks",
            "bs_balance_exec_times", "bs_balance_makespan", "bs_balance_n_microbatches",
            "bs_balance_microbatch", "bs_balance_destroy", "bs_attn_workspace_bytes", "bs_attn_fwd",
-           "bs_attn_bwd_prep", "bs_attn_bwd", "bs_attn_bwd_finish", "bs_lse_merge",
+           "bs_attn_bwd_prep", "bs_attn_bwd", "bs_attn_bwd_finish", "bs_lse_merge", "bs_softmax_xent",
            "bs_launch_count", "bs_launch_count_reset"]
 
 
@@ -287,6 +288,15 @@ def lse_merge(O_parts, LSE_parts, shape, rows, O_out, LSE_out):
     lp = (_vp * n)(*[t.data_ptr() for t in LSE_parts])
     _check(lib.bs_lse_merge(n, op, lp, ctypes.byref(shape), rows[0], rows[1], _ptr(O_out),
                             _ptr(LSE_out), _stream()), "bs_lse_merge")
+
+
+def softmax_xent(logits, labels, grad_scale, loss, dlogits, vocab=None):
+    """bs_softmax_xent on torch device tensors: logits / dlogits bf16 [T, row_stride], labels
+    int32 [T], loss fp32 [T]; vocab defaults to the row width."""
+    T, stride = logits.shape
+    _check(lib.bs_softmax_xent(_ptr(logits), _ptr(labels), T, stride if vocab is None else vocab,
+                               stride, float(grad_scale), _ptr(loss), _ptr(dlogits), _stream()),
+           "bs_softmax_xent")
 
 
 def launch_count():
