@@ -287,6 +287,11 @@ def run_ours(args, rank, world, local_rank):
         hdp_lens = RP.global_batch(w.seed, HDP_N_SHORT, HDP_CAPACITY, HDP_LONG_MULTIPLES)
         hdp = RP.replay(hdp_lens, HDP_CAPACITY, HDP_RANKS, Hq, Hkv, D, seed=w.seed)
         hdp_bal = RP.replay_balanced(hdp_lens, HDP_CAPACITY, HDP_RANKS, Hq, Hkv, D, seed=w.seed)
+        # the static-CP packed baseline on the same global batch, and whether
+        # the O(S^2) compute hides the O(S) PCIe copies of an activation offload
+        static_cp = RP.static_cp_baseline(hdp_lens, HDP_CAPACITY, HDP_RANKS, HDP_RANKS, Hq, Hkv, D,
+                                          seed=w.seed)
+        offload = RP.offload_probe((8192, 32768, 65536), Hq, Hkv, D, seed=w.seed)
         hdp["workload"] = (f"{HDP_N_SHORT} log-normal short sequences + long ones of "
                            f"{list(HDP_LONG_MULTIPLES)} x capacity, capacity {HDP_CAPACITY} tokens, "
                            f"d_hdp {HDP_RANKS}, {Hq} heads, D {D}")
@@ -315,6 +320,8 @@ def run_ours(args, rank, world, local_rank):
             "ring_steps_cfg3_4_5": ring,
             "hdp_naive_replay": hdp,
             "hdp_balance_replay": hdp_bal,
+            "static_cp_baseline": static_cp,
+            "offload_probe": offload,
             "cpu_baseline": {"value": fl / dt / 1e12, "unit": "TFLOP/s", "cores": thr, "kind": "oracle",
                              "sample": f"{CPU_BASELINE_HEADS} of {Hq} heads of {WORKLOAD}, all "
                                        f"{rows} tokens, fwd+bwd, fp64, {dt:.1f} s"},

@@ -26,12 +26,13 @@ def global_batch(seed, n_short, capacity, long_multiples):
     return [lens[int(i)] for i in perm]
 
 
-def _run_microbatch(seqs, Hq, Hkv, D, gen):
-    """One micro-batch on this GPU; returns (milliseconds, visible pairs per head)."""
+def _prepare_step(seqs, Hq, Hkv, D, gen, out):
+    """Buffers and the step closure of one micro-batch: out[0] = step, returns visible pairs."""
     pl = B.plan([(s[0], s[1], s[2]) for s in seqs])
     rows, n_steps = pl["q_rows"], pl["n_steps"]
     if rows == 0:
-        return 0.0, 0
+        out[0] = None
+        return 0
     dev = "cuda"
     Q = torch.randn(rows, Hq, D, device=dev, generator=gen).bfloat16()
     dO = torch.randn(rows, Hq, D, device=dev, generator=gen).bfloat16()
@@ -68,13 +69,23 @@ def _run_microbatch(seqs, Hq, Hkv, D, gen):
         B.attn_bwd_finish(shapes[0], acc, dQ)
 
     step()  # warm-up (first touch of the buffers)
+    out[0] = step
+    return sum(st["visible_pairs"] for st in pl["steps"])
+
+
+def _run_microbatch(seqs, Hq, Hkv, D, gen):
+    """One micro-batch on this GPU; returns (milliseconds, visible pairs per head)."""
+    holder = [None]
+    pairs = _prepare_step(seqs, Hq, Hkv, D, gen, holder)
+    if holder[0] is None:
+        return 0.0, 0
     torch.cuda.synchronize()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record()
-    step()
+    holder[0]()
     b.record()
     torch.cuda.synchronize()
-    return a.elapsed_time(b), sum(st["visible_pairs"] for st in pl["steps"])
+    return a.elapsed_time(b), pairs
 
 
 def replay(lens, capacity, d_hdp, n_q_heads, n_kv_heads, head_dim, seed=0):
@@ -179,3 +190,87 @@ def replay_balanced(lens, capacity, d_hdp, n_q_heads, n_kv_heads, head_dim, seed
                          "max_over_min": round(float(t.max() / t.min()), 2) if float(t.min()) > 0 else None,
                          "idle_frac": round(1.0 - sum(busy) / (float(t.max()) * d_hdp), 3)},
             "n_microbatches": len(bal["microbatches"])}
+
+
+def static_cp_baseline(lens, capacity, cp, d_hdp, n_q_heads, n_kv_heads, head_dim, seed=0):
+    """The static parallelism HDP replaces (Fig. 14): the batch is packed into
+    sequences of up to cp * capacity tokens, and EVERY document of a packed sequence is cut 2 cp
+    ways over a CP group of cp ranks, however short it is.  Ranks of a group are symmetric
+    (zigzag), so rank 0's micro-batch is run and timed for every packed sequence; the d_hdp / cp
+    groups take the packed sequences round-robin.  Compute only: the ring exchange, which is
+    what static CP wastes most on short documents, is outside this path."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("replay needs a CUDA device (there is no CPU path)")
+    packs, room = [[]], cp * capacity
+    for s in sorted(lens, reverse=True):          # first-fit decreasing into cp * capacity tokens
+        for pk in packs:
+            if sum(pk) + s <= room:
+                pk.append(s)
+                break
+        else:
+            packs.append([s])
+    packs = [pk for pk in packs if pk]
+    gen = torch.Generator(device="cuda").manual_seed(seed)
+    groups = max(1, d_hdp // cp)
+    group_ms = [0.0] * groups
+    pairs, rows = 0, 0
+    for k, pk in enumerate(packs):
+        ms, p = _run_microbatch([(s, cp, 0, i) for i, s in enumerate(pk)], n_q_heads, n_kv_heads,
+                                head_dim, gen)
+        group_ms[k % groups] += ms
+        pairs += p
+        rows += sum(pk) // cp
+    busy = sum(group_ms)
+    return {"cp": cp, "n_packed_sequences": len(packs), "groups": groups,
+            "rank_ms": round(max(group_ms), 3),
+            "tflops_per_rank": round(14.0 * head_dim * n_q_heads * pairs / (busy * 1e-3) / 1e12, 1)
+            if busy > 0 else None}
+
+
+def offload_probe(seq_lens, n_q_heads, n_kv_heads, head_dim, seed=0):
+    """"the O(S^2) computation time will inevitably surpass the O(S) data transfer
+    time".  For one whole sequence of S tokens: fwd+bwd compute time, the time to copy its Q, K, V
+    and O (the activations an act_ctx would offload) to pinned host memory and back, and both at
+    once on separate streams (the copies use the DMA engines)."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("the probe needs a CUDA device")
+    out = []
+    gen = torch.Generator(device="cuda").manual_seed(seed)
+    side = torch.cuda.Stream()
+    for S in seq_lens:
+        elems = S * (2 * n_q_heads + 2 * n_kv_heads) * head_dim      # Q, O, K, V
+        dev = torch.empty(elems, dtype=torch.bfloat16, device="cuda")
+        host = torch.empty(elems, dtype=torch.bfloat16, pin_memory=True)
+
+        def copies():
+            host.copy_(dev, non_blocking=True)       # D2H (forward: offload)
+            dev.copy_(host, non_blocking=True)       # H2D (backward: reload)
+
+        def timed(fn):
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b)
+        compute_ms, _ = _run_microbatch([(S, 1, 0, 0)], n_q_heads, n_kv_heads, head_dim, gen)
+        copies()
+        copy_ms = timed(copies)
+
+        def both():
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                copies()
+            _run_once[0]()
+            torch.cuda.current_stream().wait_stream(side)
+        # one more micro-batch run whose step we can call again
+        _run_once = [None]
+        _prepare_step([(S, 1, 0, 0)], n_q_heads, n_kv_heads, head_dim, gen, _run_once)
+        both_ms = timed(both)
+        out.append({"tokens": S, "compute_ms": round(compute_ms, 3), "copy_ms": round(copy_ms, 3),
+                    "both_ms": round(both_ms, 3), "bytes_each_way": elems * 2,
+                    "overlap": round(max(compute_ms, copy_ms) / both_ms, 3),   # 1.0 = perfect
+                    "copy_hidden_by_compute": compute_ms >= copy_ms})
+        del dev, host
+    return out

@@ -35,3 +35,16 @@ def test_balanced_replay_of_a_small_global_batch():
     m = r["measured"]
     assert len(m["rank_finish_ms"]) == d_hdp and m["min_ms"] <= m["max_ms"]
     assert 0.0 <= m["idle_frac"] < 1.0
+
+
+def test_static_cp_baseline_and_offload_probe():
+    cap, d_hdp = 512, 4
+    lens = RP.global_batch(3, 24, cap, (3, 2))
+    r = RP.static_cp_baseline(lens, cap, 4, d_hdp, 4, 2, 64, seed=3)
+    assert r["cp"] == 4 and r["groups"] == 1 and r["rank_ms"] > 0
+    assert r["n_packed_sequences"] >= -(-sum(lens) // (4 * cap))
+    o = RP.offload_probe((1024, 4096), 4, 2, 64, seed=3)
+    assert [x["tokens"] for x in o] == [1024, 4096]
+    for x in o:
+        assert x["compute_ms"] > 0 and x["copy_ms"] > 0 and x["both_ms"] > 0
+        assert x["bytes_each_way"] == x["tokens"] * (2 * 4 + 2 * 2) * 64 * 2
