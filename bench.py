@@ -281,6 +281,7 @@ def run_ours(args, rank, world, local_rank):
         merge = bench_merge(B, torch, pk)
         xent = bench_softmax_xent(B, torch, pk)
         ring = bench_ring_steps(B, torch, workloads, pk)
+        full = bench_full_configs(B, torch, workloads, pk)
         # naive HDP assignment (bs_assign) of a synthetic global batch,
         # every rank's micro-batches replayed on this GPU
         from paper_2502_21231_b200 import replay as RP
@@ -318,6 +319,7 @@ def run_ours(args, rank, world, local_rank):
             "merge": merge,
             "softmax_xent": xent,
             "ring_steps_cfg3_4_5": ring,
+            "full_configs": full,
             "hdp_naive_replay": hdp,
             "hdp_balance_replay": hdp_bal,
             "static_cp_baseline": static_cp,
@@ -387,6 +389,88 @@ def bench_softmax_xent(B, torch, pk):
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s",
                          "frac": gbs / pk["hbm"], "frac_of_nominal_8000": gbs / 8000.0,
                          "traffic": ncu_traffic("softmax_xent")}}
+
+
+def bench_full_configs(B, torch, workloads, pk, cfgs=(1, 3, 4, 5)):
+    """every config as a WHOLE pipeline on seeded-shape random device data - all ring
+    steps of bs_attn_fwd (the first one clears dQ_acc), bs_lse_merge over all partials, prep, all
+    ring steps of bs_attn_bwd, finish - each phase timed once with CUDA events after one untimed
+    warm-up pass of the same launches.  cfg1 is forward only and latency-bound: microseconds."""
+    out = {}
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+    for cfg in cfgs:
+        w = workloads.make_workload(cfg)
+        pl = B.plan(w.seqs)
+        Hq, Hkv, D, rows, n = w.n_q_heads, w.n_kv_heads, w.head_dim, pl["q_rows"], pl["n_steps"]
+        Q = torch.randn(rows, Hq, D, device="cuda").bfloat16()
+        dO = torch.randn_like(Q)
+        acc = torch.empty((rows, Hq, D), dtype=torch.float32, device="cuda")
+        steps = []
+        for st in pl["steps"]:
+            K = torch.randn(st["kv_rows"], Hkv, D, device="cuda").bfloat16()
+            sh = B.make_shape(Hq, Hkv, D, rows, st["kv_rows"])
+            nb = max(B.attn_workspace_bytes(sh, len(st["segs"]), False),
+                     B.attn_workspace_bytes(sh, len(st["segs"]), True))
+            steps.append(dict(st=st, sh=sh, K=K, V=torch.randn_like(K), dK=torch.empty_like(K),
+                              dV=torch.empty_like(K), O=torch.empty_like(Q),
+                              L=torch.empty((Hq, rows), dtype=torch.float32, device="cuda"),
+                              ws=torch.empty(nb, dtype=torch.uint8, device="cuda")))
+        sh0 = steps[0]["sh"]
+        # merged rows: the rows that take part in more than one step (cfg4: the long shard only)
+        m_end = max(sg[1] for d in steps[1:] for sg in d["st"]["segs"]) if n > 1 else 0
+        # running merge: the output aliases part 0 (include/bytescale_attn.h), so rows that are
+        # final after step 0 (cfg4's short documents) need no copy
+        O, LSE = steps[0]["O"], steps[0]["L"]
+        delta = torch.empty_like(LSE)
+        dQ = torch.empty_like(Q)
+
+        def fwd():
+            for i, d in enumerate(steps):
+                B.attn_fwd(d["sh"], Q, d["K"], d["V"], d["st"]["segs"], (0, rows if i == 0 else m_end),
+                           d["O"], d["L"], d["ws"], acc if i == 0 else None)
+
+        def merge():
+            if n > 1:
+                B.lse_merge([d["O"] for d in steps], [d["L"] for d in steps], sh0, (0, m_end), O, LSE)
+
+        def bwd():
+            B.attn_bwd_prep(sh0, O, dO, delta, None)
+            for d in steps:
+                B.attn_bwd(d["sh"], Q, d["K"], d["V"], dO, LSE, delta, d["st"]["segs"], acc, d["dK"],
+                           d["dV"], d["ws"])
+            B.attn_bwd_finish(sh0, acc, dQ)
+
+        phases = (fwd,) if cfg == 1 else (fwd, merge, bwd)
+        reps = 20 if cfg == 1 else 1
+        for f in phases:  # warm-up pass
+            f()
+        torch.cuda.synchronize()
+        t = []
+        for f in phases:
+            a, b = ev(), ev()
+            a.record()
+            for _ in range(reps):
+                f()
+            b.record()
+            torch.cuda.synchronize()
+            t.append(a.elapsed_time(b) / reps)
+        pairs = sum(st["visible_pairs"] for st in pl["steps"])
+        if cfg == 1:
+            out["cfg1"] = {"fwd_us": round(1e3 * t[0], 2), "visible_pairs_per_head": pairs,
+                           "note": "latency-bound correctness config: 960 tokens, 4 heads, D 64"}
+            continue
+        mbytes = (n + 1) * m_end * Hq * (2 * D + 4)
+        both = 14.0 * D * Hq * pairs / (t[0] + t[2]) / 1e9
+        out[f"cfg{cfg}"] = {
+            "ring_steps": n, "visible_pairs_per_head": pairs,
+            "fwd_ms": round(t[0], 3), "merge_ms": round(t[1], 3), "bwd_ms": round(t[2], 3),
+            "fwd_tflops": round(4.0 * D * Hq * pairs / t[0] / 1e9, 1),
+            "bwd_tflops": round(10.0 * D * Hq * pairs / t[2] / 1e9, 1),
+            "fwd_bwd_tflops": round(both, 1), "frac_of_measured_peak": round(both / pk["tflops"], 3),
+            "merge_gbs": round(mbytes / t[1] / 1e6, 1), "merge_bytes": mbytes}
+        del steps, Q, dO, acc, O, LSE, delta, dQ
+        torch.cuda.empty_cache()
+    return out
 
 
 def bench_ring_steps(B, torch, workloads, pk):
