@@ -56,6 +56,46 @@ __device__ __forceinline__ uint32_t pack2(float lo, float hi) {
   return *reinterpret_cast<uint32_t*>(&t);
 }
 
+// phase 2 of the merge for n_parts <= kNP: kU outputs per thread and pass
+template <int kVecPerHead, int kU, int kNP>
+__device__ __forceinline__ void merge_few(const MergeParams& p, const float* w_smem, int row0, int h0,
+                                          int nrows, int vec_per_row) {
+  const int n = p.n_parts, total = nrows * vec_per_row;
+  for (int t0 = threadIdx.x; t0 < total; t0 += blockDim.x * kU) {
+    uint4 v[kU][kNP];
+    int64_t off[kU];
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+      const int t = t0 + u * blockDim.x;
+      const int r = t / vec_per_row, c = t % vec_per_row;
+      off[u] = (int64_t)(row0 + r) * p.row_stride_v + (int64_t)h0 * kVecPerHead + c;
+#pragma unroll
+      for (int j = 0; j < kNP; ++j)
+        if (t < total && j < n) v[u][j] = ldg_stream(p.O_parts[j] + off[u]);
+    }
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+      const int t = t0 + u * blockDim.x;
+      if (t >= total) break;
+      const int r = t / vec_per_row, h = (t % vec_per_row) / kVecPerHead;
+      float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int j = 0; j < kNP; ++j) {
+        if (j < n) {
+          const float w = w_smem[(j * kRowsPerTile + r) * p.heads_per_block + h];
+          if (w != 0.f) fma_bf16x8(acc, v[u][j], w);  // zero weight: the part may hold NaN
+        }
+      }
+      uint4 o;
+      o.x = pack2(acc[0], acc[1]);
+      o.y = pack2(acc[2], acc[3]);
+      o.z = pack2(acc[4], acc[5]);
+      o.w = pack2(acc[6], acc[7]);
+      stg_stream(p.O_out + off[u], o);
+    }
+  }
+}
+
 // grid: (row tiles, head slabs).  smem: weights[n_parts][kRowsPerTile][heads_per_block] fp32.
 template <int kVecPerHead>  // uint4 per (row, head): D / 8
 __global__ void __launch_bounds__(kStreamThreads) lse_merge_kernel(const __grid_constant__ MergeParams p) {
@@ -88,6 +128,16 @@ __global__ void __launch_bounds__(kStreamThreads) lse_merge_kernel(const __grid_
 
   // phase 2: stream O.  Within a row the slab's heads are contiguous: nh * kVecPerHead uint4.
   const int vec_per_row = nh * kVecPerHead;
+  // few parts (a running merge, n = 2): one output per thread keeps only n 16-byte loads in
+  // flight; take kU outputs per thread and pass so that every thread has 8 loads in flight
+  // (16 loads per thread cost 98 registers instead of 64 and every case got slower: measured)
+  if (n <= 4) {
+    if (n <= 2)
+      merge_few<kVecPerHead, 4, 2>(p, w_smem, row0, h0, nrows, vec_per_row);
+    else
+      merge_few<kVecPerHead, 2, 4>(p, w_smem, row0, h0, nrows, vec_per_row);
+    return;
+  }
   for (int t = threadIdx.x; t < nrows * vec_per_row; t += blockDim.x) {
     const int r = t / vec_per_row, c = t % vec_per_row;
     const int h = c / kVecPerHead;
@@ -297,6 +347,7 @@ bs_status_t bs_lse_merge(int32_t n_parts, const void* const* O_parts, const floa
   p.row_stride_v = shape->q_row_stride / 8;
   p.lse_head_stride = shape->lse_head_stride;
   p.heads_per_block = pick_heads_per_block(shape->n_q_heads, n_parts, 40 * 1024);
+  if (p.heads_per_block > 32) p.heads_per_block = 32;  // smaller blocks: a smoother tail, more of them per SM
   const size_t smem = (size_t)n_parts * kRowsPerTile * p.heads_per_block * sizeof(float);
   dim3 grid((row_end - row_begin + kRowsPerTile - 1) / kRowsPerTile,
             (shape->n_q_heads + p.heads_per_block - 1) / p.heads_per_block);
