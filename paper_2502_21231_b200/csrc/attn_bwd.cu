@@ -290,11 +290,13 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       // unit's last dP^T MMA and K at its last dQ MMA.  K/V then stream in under the previous
       // unit's tail (dS, dK/dQ, the dQ drain and the dK/dV epilogue).
       auto load_kv = [&]() {
+        TRACE(2, 8, it_n);  // the producer is ready to load this unit's K / V
         mbar_wait(v_empty, (item_n & 1) ^ 1);
         mbar_arrive_expect_tx(v_full, L::kTileBytes);
         for (int half = 0; half < D / 64; ++half)
           tma_load_3d(smem + L::kVOff + half * (kTile * 128), &tmV, v_full, half * 64, g, it.row0);
         mbar_wait(k_empty, (item_n & 1) ^ 1);
+        TRACE(2, 9, it_n);  // K requested
         mbar_arrive_expect_tx(k_full, L::kTileBytes);
         for (int half = 0; half < D / 64; ++half)
           tma_load_3d(smem + L::kKOff + half * (kTile * 128), &tmK, k_full, half * 64, g, it.row0);
@@ -353,10 +355,13 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         BwdWalker wk;
         wk.init(p.sv.spans, u, p.group);
         if (wk.done()) continue;
+        TRACE(2, 5, it_n);  // unit picked up
         mbar_wait(k_full, item_n & 1);
+        TRACE(2, 6, it_n);
         tc_fence_after();
         // prologue: S^T(0)
         mbar_wait(&q_full[it_n & 1], (it_n >> 1) & 1);
+        TRACE(2, 7, it_n);
         tc_fence_after();
         issue_kmajor<D>(tmem, sK, sQ + (it_n & 1) * L::kTileBytes);
         tc_commit(s_full);
