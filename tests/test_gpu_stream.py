@@ -17,7 +17,10 @@ def _imports():
 
 
 @pytest.mark.parametrize("n,rows,Hq,D", [(1, 37, 4, 64), (2, 100, 6, 128), (8, 515, 16, 128),
-                                          (64, 70, 48, 128), (5, 9, 3, 64)])
+                                          (64, 70, 48, 128), (5, 9, 3, 64),
+                                          # n <= 4: several outputs per thread and pass; more heads
+                                          # than one block owns (32), ragged last row tile
+                                          (3, 61, 40, 128), (4, 131, 64, 64), (2, 9, 33, 128)])
 def test_lse_merge_vs_oracle(nprng, n, rows, Hq, D):
     torch, B, U = _imports()
     O_bits = [randn_bf16(nprng, rows, Hq, D) for _ in range(n)]
