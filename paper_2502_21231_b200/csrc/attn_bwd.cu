@@ -84,7 +84,7 @@ struct BwdSmem {
   static constexpr int kQOff = 2 * kTileBytes;          // 2 stages
   static constexpr int kDOOff = 4 * kTileBytes;         // 1 stage
   static constexpr int kDSOff = 5 * kTileBytes;         // dS^T [128 keys][128 queries] bf16
-  static constexpr int kDQOff = kDSOff + kTile * kTile * 2;  // 2 x [128][32] fp32 staging
+  static constexpr int kDQOff = kDSOff + kTile * kTile * 2;  // 2 x [128][32] fp32 staging (dQ), 16 KB boxes
   static constexpr int kLseOff = kDQOff + 2 * kTile * 128;   // [2 stages][128] lse*log2e
   static constexpr int kDeltaOff = kLseOff + 2 * kTile * 4;  // [2 stages][128] delta*scale
   static constexpr int kBarOff = kDeltaOff + 2 * kTile * 4;
@@ -421,9 +421,12 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   } else if (warp >= 12) {
     // ===================================== dQ drain warpgroup =====================================
     // dQ of every iteration: TMEM -> registers -> shared -> TMA reduce-add (fp32 add in L2) into
-    // dQ_acc, 16 columns (one 8 KB box of 128 rows x 64 B, 64-byte swizzle) at a time through
-    // four staging boxes.  The TMA unit needs ~1300 cycles to read a box; that used to sit on the
-    // compute warps' critical path.  Only the TMEM -> register lift is urgent (see the issuer).
+    // dQ_acc, 32 columns (one 16 KB box of 128 rows x 128 B, 128-byte swizzle) at a time through
+    // two staging boxes: whole 128-byte lines per row on the way to L2 (with four 8 KB boxes of
+    // 64-byte row segments the backward was 2-3 % slower - the SM's request path to L2 is 64 %
+    // busy in this kernel, ncu l1tex__m_l1tex2xbar_req_cycles_active).  The TMA unit needs well
+    // over 1000 cycles to read a box; that used to sit on the compute warps' critical path.  Only
+    // the TMEM -> register lift is urgent (see the issuer).
     setmaxnreg_inc<kRegsDrain>();
     const int r = threadIdx.x & 127;  // query row of the tile
     const uint32_t tY = tmem + (uint32_t((warp & 3) * 32) << 16) + 128;
@@ -448,19 +451,19 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         tc_fence_before();
         warp_arrive(dq_drained);
 #pragma unroll
-        for (int c = 0; c < D / 16; ++c) {
-          uint8_t* stage = stage0 + (c & 3) * 8192;
-          if (r == 0) bulk_wait_group_read<3>();  // the reduce four chunks back has read this box
+        for (int c = 0; c < D / 32; ++c) {
+          uint8_t* stage = stage0 + (c & 1) * 16384;
+          if (r == 0) bulk_wait_group_read<1>();  // the reduce two chunks back has read this box
           bar_sync(3, 128);
 #pragma unroll
-          for (int j = 0; j < 4; ++j)
-            *reinterpret_cast<uint4*>(stage + r * 64 + ((j ^ ((r >> 1) & 3)) * 16)) =
-                make_uint4(v[16 * c + 4 * j], v[16 * c + 4 * j + 1], v[16 * c + 4 * j + 2],
-                           v[16 * c + 4 * j + 3]);
+          for (int j = 0; j < 8; ++j)
+            *reinterpret_cast<uint4*>(stage + r * 128 + ((j ^ (r & 7)) * 16)) =
+                make_uint4(v[32 * c + 4 * j], v[32 * c + 4 * j + 1], v[32 * c + 4 * j + 2],
+                           v[32 * c + 4 * j + 3]);
           fence_proxy_async_smem();
           bar_sync(3, 128);
           if (r == 0) {
-            tma_reduce_add_3d(&tmDQ, stage, c * 16, h, qrow);
+            tma_reduce_add_3d(&tmDQ, stage, c * 32, h, qrow);
             bulk_commit_group();
           }
         }
@@ -711,7 +714,7 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
                               shape->kv_row_stride, 64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmDQ, dQ_acc, 4, D, shape->n_q_heads, shape->q_rows,
-                              (int64_t)shape->n_q_heads * D, 16, bs::kTile, 64);
+                              (int64_t)shape->n_q_heads * D, 32, bs::kTile, 128);
   if (rc != BS_OK) return rc;
 
   rc = bs::make_tensor_map_3d(&tmDK, dK, 2, D, shape->n_kv_heads, shape->kv_rows,
