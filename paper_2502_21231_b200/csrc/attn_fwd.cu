@@ -437,13 +437,9 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint32_t s_ph = 0, o_ph = 0;
     int tr_it = 0;
     UnitConsumer cons{sched};
-    // The next unit is taken from the scheduler ring BEFORE the epilogue's stores: 64 row-per-thread
-    // store instructions per unit touch 32 lines each and hold the LSU for ~2000 cycles, and the
-    // shared-memory reads of the pick-up would queue behind them (clock64 trace: 1000-1600 cycles).
-    Unit u, u_next;
-    bool more = cons.next(&u);
+    Unit u;
     int un = -1;
-    for (; more; u = u_next) {
+    while (cons.next(&u)) {
       ++un;
       if (r == 0 && hf == 0) UTRACE(t, 0, un);
       const Item& it = u.item;
@@ -456,7 +452,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       __nv_bfloat16* o_ptr = p.O + grow * p.o_row_stride + (int64_t)h * D + hf * (D / 2);
       const int tot = wk.total(t);
       if (tot == 0) {  // no key of this call is visible to any row of the tile
-        more = cons.next(&u_next);
         if (valid) {
           for (int c = 0; c < D / 16; ++c) reinterpret_cast<uint4*>(o_ptr)[c] = make_uint4(0, 0, 0, 0);
           if (hf == 0) p.LSE[(int64_t)h * p.lse_head_stride + grow] = -CUDART_INF_F;
@@ -626,7 +621,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       o_ph ^= 1;
       if (r == 0 && hf == 0) UTRACE(t, 3, un);
       tc_fence_after();
-      more = cons.next(&u_next);
       const float inv_l = l > 0.f ? 1.f / l : 0.f;
 #pragma unroll
       for (int c = 0; c < D / 32; ++c) {
