@@ -42,11 +42,20 @@ namespace {
 using namespace bs;
 using namespace bs::ptx;
 
+#ifndef BS_SCHED_SLOTS
+#define BS_SCHED_SLOTS 1
+#endif
+constexpr int kBwdSchedSlots = BS_SCHED_SLOTS;  // depth of the scheduler ring (sched.cuh)
+using SchedRing = SchedRingT<kBwdSchedSlots>;
+using UnitProducer = UnitProducerT<kBwdSchedSlots>;
+using UnitConsumer = UnitConsumerT<kBwdSchedSlots>;
+constexpr int kSchedRingBytes = SchedRing::kBytes;
+
 constexpr int kBwdThreads = 512;   // 2 compute WGs, auxiliary WG (MMA, TMA, scheduler), dQ drain WG
 constexpr int kRegsCompute = 144, kRegsAux = 64, kRegsDrain = 160;  // 2*144 + 64 + 160 = 4*128
 constexpr int kComputeThreads = 256;
 #ifndef BS_BWD_EMU
-#define BS_BWD_EMU 1
+#define BS_BWD_EMU 0  // (1 of 4 was worth ~1 % before the dQ boxes became whole lines; now 0 is 2 % faster on cfg2)
 #endif
 constexpr int kBwdEmuOf4 = BS_BWD_EMU;  // of every 4 column pairs, this many take the FMA-pipe exp2
 

@@ -30,6 +30,15 @@ namespace {
 using namespace bs;
 using namespace bs::ptx;
 
+#ifndef BS_SCHED_SLOTS
+#define BS_SCHED_SLOTS 2
+#endif
+constexpr int kFwdSchedSlots = BS_SCHED_SLOTS;  // depth of the scheduler ring (sched.cuh)
+using SchedRing = SchedRingT<kFwdSchedSlots>;
+using UnitProducer = UnitProducerT<kFwdSchedSlots>;
+using UnitConsumer = UnitConsumerT<kFwdSchedSlots>;
+constexpr int kSchedRingBytes = SchedRing::kBytes;
+
 constexpr int kFwdThreads = 640;      // 4 softmax warpgroups + 1 auxiliary warpgroup (MMA, TMA)
 constexpr int kMmaWarp0 = 16, kTmaWarp = 17, kSchedWarp = 19;  // warps 16 / 18 issue the MMAs of Q tile 0 / 1
 constexpr int kRegsSoftmax = 104;     // setmaxnreg: 512 * 104 + 128 * 96 = 65536 (compiled at 96)

@@ -47,50 +47,52 @@ __device__ __forceinline__ Unit decode_unit(const SchedView& sv, int32_t w, int3
   return u;
 }
 
-#ifndef BS_SCHED_SLOTS
-#define BS_SCHED_SLOTS 3
-#endif
-constexpr int kSchedSlots = BS_SCHED_SLOTS;
-
-struct SchedRing {  // lives in shared memory (16-byte aligned)
-  Item item[kSchedSlots];  // decoded by the producer: consumers never touch the global tables
-  Span sp[kSchedSlots][2];
-  int32_t head[kSchedSlots];
-  int32_t unit[kSchedSlots];
-  uint64_t full[kSchedSlots], empty[kSchedSlots];
+// kSlots = depth of the ring = how far the scheduler warp may run ahead of the slowest role.  A
+// claimed unit cannot move to another CTA any more, so less look-ahead means later binding and a
+// better balance; measured on cfg2 (3 -> 2 -> 1 slots): forward 0.695 -> 0.688 -> 0.692 ms,
+// backward 1.569 -> 1.549 -> 1.517 ms; 4 slots are slower than 3 in both.  The kernels choose.
+template <int kSlots>
+struct SchedRingT {  // lives in shared memory (16-byte aligned)
+  Item item[kSlots];  // decoded by the producer: consumers never touch the global tables
+  Span sp[kSlots][2];
+  int32_t head[kSlots];
+  int32_t unit[kSlots];
+  uint64_t full[kSlots], empty[kSlots];
+  static constexpr int kBytes = 128 * kSlots;
 };
-constexpr int kSchedRingBytes = 128 * kSchedSlots;
-static_assert(sizeof(SchedRing) <= kSchedRingBytes, "SchedRing size");
 
 // n_consumers = arrivals per slot on the empty barrier (threads calling next(), warps calling
 // next_warp())
-__device__ __forceinline__ void sched_ring_init(SchedRing* r, uint32_t n_consumers) {
-  for (int i = 0; i < kSchedSlots; ++i) {
+template <int kSlots>
+__device__ __forceinline__ void sched_ring_init(SchedRingT<kSlots>* r, uint32_t n_consumers) {
+  static_assert(sizeof(SchedRingT<kSlots>) <= SchedRingT<kSlots>::kBytes, "SchedRing size");
+  for (int i = 0; i < kSlots; ++i) {
     ptx::mbar_init(&r->full[i], 1);
     ptx::mbar_init(&r->empty[i], n_consumers);
   }
 }
 
-struct UnitProducer {  // one thread (the scheduler warp's lane 0)
-  SchedRing* r;
+template <int kSlots>
+struct UnitProducerT {  // one thread (the scheduler warp's lane 0)
+  SchedRingT<kSlots>* r;
   uint32_t n = 0;
   int32_t hint = 0, last = 0;
   // Pulls the next unit of this CTA from the global cursor, decodes it and publishes it.
   // Returns false when the cursor ran out (also published, as unit -1).
-  // Look-ahead: up to kSchedSlots - 1 units beyond the one the slowest consumer works on while
+  // Look-ahead: up to kSlots - 1 units beyond the one the slowest consumer works on while
   // plenty of units are left; once the cursor is within 4 rounds of the end a unit is only
   // claimed when every consumer has taken the previous one, so that the short tail units go to
   // whichever CTA is free first (greedy longest-first).
   __device__ __forceinline__ bool next(const SchedView& sv, Unit* u) {
     if (n > 0 && last >= sv.n_units - 4 * (int32_t)gridDim.x) {
-      const uint32_t pslot = (n - 1) % kSchedSlots, pph = ((n - 1) / kSchedSlots) & 1;
+      const uint32_t pslot = (n - 1) % kSlots, pph = ((n - 1) / kSlots) & 1;
       ptx::mbar_wait(&r->empty[pslot], pph);
     }
     int32_t w = atomicAdd(sv.counter, 1);
     last = w;
     if (w >= sv.n_units) w = -1;
     if (w >= 0) *u = decode_unit(sv, w, &hint);
-    const uint32_t slot = n % kSchedSlots, ph = (n / kSchedSlots) & 1;
+    const uint32_t slot = n % kSlots, ph = (n / kSlots) & 1;
     ptx::mbar_wait(&r->empty[slot], ph ^ 1);
     if (w >= 0) {
       r->item[slot] = u->item;
@@ -112,11 +114,12 @@ __device__ __forceinline__ T warp_uniform(T v) {
   return __shfl_sync(0xffffffffu, v, 0);
 }
 
-struct UnitConsumer {  // every consuming thread
-  SchedRing* r;
+template <int kSlots>
+struct UnitConsumerT {  // every consuming thread
+  SchedRingT<kSlots>* r;
   uint32_t n = 0;
   __device__ __forceinline__ bool next(Unit* u) {
-    const uint32_t slot = n % kSchedSlots, ph = (n / kSchedSlots) & 1;
+    const uint32_t slot = n % kSlots, ph = (n / kSlots) & 1;
     ptx::mbar_wait(&r->full[slot], ph);
     const int32_t w = r->unit[slot];
     if (w >= 0) {
@@ -132,7 +135,7 @@ struct UnitConsumer {  // every consuming thread
   // Wait for slot n and read it without consuming it (lanes 1-31 of a warp whose lane 0
   // consumes for the warp afterwards).
   __device__ __forceinline__ void wait_peek(Unit* u) const {
-    const uint32_t slot = n % kSchedSlots, ph = (n / kSchedSlots) & 1;
+    const uint32_t slot = n % kSlots, ph = (n / kSlots) & 1;
     ptx::mbar_wait(&r->full[slot], ph);
     u->item = r->item[slot];
     u->head = r->head[slot];
