@@ -202,6 +202,24 @@ __device__ __forceinline__ void warp_arrive(uint64_t* bar) {
   if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
 }
 
+// Rows [v, 128) of a 128-row tile (TMA layout: one 16 KB box of 128-byte rows per 64 columns) are
+// set to zero by the 256 compute threads.  TMA loads whole boxes, so behind a ragged range end the
+// tile holds whatever follows in the caller's buffer - another document, or uninitialised rows
+// with NaN / Inf.  Masked P and dS are exactly 0, but 0 x NaN inside an MMA's contraction would
+// still poison every output row of the tile; the rows a contraction runs over must be finite.
+// (The 128-byte swizzle permutes 16-byte chunks inside a row: zeroing whole rows needs no index
+// arithmetic.)
+template <int D>
+__device__ __forceinline__ void zero_tile_rows(uint8_t* tile, int v, int tid256) {
+  constexpr int kChunksPerRow = D / 8;  // 16-byte chunks of one row over all column boxes
+  const int total = (kTile - v) * kChunksPerRow;
+  for (int i = tid256; i < total; i += kComputeThreads) {
+    const int row = v + i / kChunksPerRow, cc = i % kChunksPerRow;
+    *reinterpret_cast<uint4*>(tile + (cc / 8) * (kTile * 128) + row * 128 + (cc % 8) * 16) =
+        make_uint4(0, 0, 0, 0);
+  }
+}
+
 template <int D>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
@@ -508,6 +526,10 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       }
       uint32_t pk[32];  // P^T of this thread as the tensor core sees it (bf16 pairs), kept for dS
       bool first = true;
+      bool full_it = false;      // mask of the current iteration, kept for the dS step
+      int c_min_it = 0, c_max_it = 0;
+      const int tid256 = threadIdx.x & 255;
+      const int vk = it.range_len - it.local0;  // valid keys of the tile (>= 128: all)
 
       auto compute_p = [&](const BwdWalker& k, uint32_t n) {
         mbar_wait(s_full, n & 1);
@@ -525,6 +547,28 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                           a0 + 64 <= k.sp.len;
         const int c_min = key_ok ? b - k.sp.off - a0 : (1 << 30);
         const int c_max = k.sp.len - a0;
+        full_it = full;
+        c_min_it = c_min;
+        c_max_it = c_max;
+        // Ragged tiles: rows past the range end must not carry NaN / Inf into a contraction.
+        // K rows past the key range (the dQ MMA sums over keys): once per unit, K has landed
+        // (S^T of this iteration is complete).  Q and dO rows past the query range (the dK and dV
+        // MMAs sum over queries): Q has landed with S^T; dO's own barrier is awaited here, the dV
+        // MMA waits for this warp's p_full arrival below.  S^T / dP^T themselves are elementwise
+        // in those rows and masked by select.
+        bool zeroed = false;
+        if (first && vk < kTile) {
+          zero_tile_rows<D>(smem + L::kKOff, vk, tid256);
+          zeroed = true;
+        }
+        const int vq = k.sp.len - k.qi * kTile;  // valid queries of the tile (>= 128: all)
+        if (vq < kTile) {
+          mbar_wait(do_full, n & 1);
+          zero_tile_rows<D>(smem + L::kQOff + (n & 1) * L::kTileBytes, vq, tid256);
+          zero_tile_rows<D>(smem + L::kDOOff, vq, tid256);
+          zeroed = true;
+        }
+        if (zeroed) fence_proxy_async_smem();
         const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
         // two copies of the loop: unmasked pieces (nearly all of them) run branch- and
         // predicate-free straight-line code
@@ -572,21 +616,30 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           }
           const float2* nd2 = reinterpret_cast<const float2*>(delta_s + (it_n & 1) * kTile + wg * 64);
           const float2 s2 = make_float2(p.scale, p.scale);
+          // two copies, as for P: masked pieces build dS by select (P = 0 times a dP from rows
+          // past a range end - possibly NaN - must give 0), unmasked ones stay straight-line code
+          auto ds_all = [&](auto masked) {
 #pragma unroll
-          for (int j = 0; j < 8; ++j) {  // 8 queries = one 16-byte chunk of the dS^T row
-            uint32_t w4[4];
+            for (int j = 0; j < 8; ++j) {  // 8 queries = one 16-byte chunk of the dS^T row
+              uint32_t w4[4];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const int i = 4 * j + e;
-              const float2 t = fma2(make_float2(__uint_as_float(dp[2 * i]), __uint_as_float(dp[2 * i + 1])),
-                                    s2, nd2[i]);
-              // P widened exactly from the bf16 pair the dV MMA used
-              const float2 d = mul2(make_float2(__uint_as_float(pk[i] << 16),
-                                                __uint_as_float(pk[i] & 0xffff0000u)), t);
-              w4[e] = pack_bf16(d.x, d.y);
+              for (int e = 0; e < 4; ++e) {
+                const int i = 4 * j + e;
+                const float2 t = fma2(make_float2(__uint_as_float(dp[2 * i]), __uint_as_float(dp[2 * i + 1])),
+                                      s2, nd2[i]);
+                // P widened exactly from the bf16 pair the dV MMA used
+                float2 d = mul2(make_float2(__uint_as_float(pk[i] << 16),
+                                            __uint_as_float(pk[i] & 0xffff0000u)), t);
+                if (decltype(masked)::value) {
+                  if (2 * i < c_min_it || 2 * i >= c_max_it) d.x = 0.f;
+                  if (2 * i + 1 < c_min_it || 2 * i + 1 >= c_max_it) d.y = 0.f;
+                }
+                w4[e] = pack_bf16(d.x, d.y);
+              }
+              *reinterpret_cast<uint4*>(ds_row + ((j ^ (r & 7)) * 16)) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
             }
-            *reinterpret_cast<uint4*>(ds_row + ((j ^ (r & 7)) * 16)) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
-          }
+          };
+          if (full_it) ds_all(std::false_type{}); else ds_all(std::true_type{});
         }
         if (r == 0) TRACE(wg, 9, it_n);
         fence_proxy_async_smem();
@@ -695,19 +748,16 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
              "bs_attn_bwd: output pointers must be 16-byte aligned");
   if (shape->kv_rows == 0) return BS_OK;
   cudaStream_t st = (cudaStream_t)stream;
+  // Everything that can fail on an argument comes first: work list, workspace, device, tensor
+  // maps (pointer / stride alignment).  Nothing is enqueued before all of it has passed.
   bs::SchedTables tb;
   rc = bs::build_bwd_tables(segs, n_segs, shape->q_rows, shape->kv_rows, shape->n_kv_heads, &tb);
   if (rc != BS_OK) return rc;
   bs::WsLayout L;
-  rc = bs::upload_tables(tb, ws, ws_bytes, st, &L);
+  rc = bs::check_workspace(tb, ws, ws_bytes, &L);
   if (rc != BS_OK) return rc;
-  uint8_t* wsb = (uint8_t*)ws;
-  rc = bs::launch_fill_rows((const int2*)(wsb + L.fill_off), (int)tb.fill.size(), tb.max_fill_rows,
-                            dK, dV, nullptr, shape->n_kv_heads, shape->head_dim,
-                            shape->kv_row_stride, 0, st);
+  rc = bs::check_device();
   if (rc != BS_OK) return rc;
-  if (tb.items.empty()) return BS_OK;
-
   const int D = shape->head_dim;
   CUtensorMap tmQ, tmK, tmV, tmDO, tmDQ, tmDK, tmDV;
   rc = bs::make_tensor_map_3d(&tmQ, Q, 2, D, shape->n_q_heads, shape->q_rows, shape->q_row_stride,
@@ -725,13 +775,21 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   rc = bs::make_tensor_map_3d(&tmDQ, dQ_acc, 4, D, shape->n_q_heads, shape->q_rows,
                               (int64_t)shape->n_q_heads * D, 32, bs::kTile, 128);
   if (rc != BS_OK) return rc;
-
   rc = bs::make_tensor_map_3d(&tmDK, dK, 2, D, shape->n_kv_heads, shape->kv_rows,
                               shape->kv_row_stride, 32, bs::kTile, 64);
   if (rc != BS_OK) return rc;
   rc = bs::make_tensor_map_3d(&tmDV, dV, 2, D, shape->n_kv_heads, shape->kv_rows,
                               shape->kv_row_stride, 32, bs::kTile, 64);
   if (rc != BS_OK) return rc;
+
+  rc = bs::upload_tables(tb, L, ws, st);
+  if (rc != BS_OK) return rc;
+  uint8_t* wsb = (uint8_t*)ws;
+  rc = bs::launch_fill_rows((const int2*)(wsb + L.fill_off), (int)tb.fill.size(), tb.max_fill_rows,
+                            dK, dV, nullptr, shape->n_kv_heads, shape->head_dim,
+                            shape->kv_row_stride, 0, st);
+  if (rc != BS_OK) return rc;
+  if (tb.items.empty()) return BS_OK;
 
   BwdParams p;
   p.sv = bs::make_sched_view(wsb, L, tb, shape->n_kv_heads);
@@ -750,12 +808,12 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   p.n_q_heads = shape->n_q_heads;
   const int grid = tb.n_units < bs::sm_count() ? tb.n_units : bs::sm_count();
   if (D == 128) {
-    BS_CUDA(cudaFuncSetAttribute(attn_bwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 BwdSmem<128>::kBytes));
+    rc = bs::set_max_smem_once((const void*)attn_bwd_kernel<128>, BwdSmem<128>::kBytes, 2);
+    if (rc != BS_OK) return rc;
     attn_bwd_kernel<128><<<grid, kBwdThreads, BwdSmem<128>::kBytes, st>>>(tmQ, tmK, tmV, tmDO, tmDQ, tmDK, tmDV, p);
   } else {
-    BS_CUDA(cudaFuncSetAttribute(attn_bwd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 BwdSmem<64>::kBytes));
+    rc = bs::set_max_smem_once((const void*)attn_bwd_kernel<64>, BwdSmem<64>::kBytes, 3);
+    if (rc != BS_OK) return rc;
     attn_bwd_kernel<64><<<grid, kBwdThreads, BwdSmem<64>::kBytes, st>>>(tmQ, tmK, tmV, tmDO, tmDQ, tmDK, tmDV, p);
   }
   BS_CUDA(cudaGetLastError());

@@ -445,6 +445,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
     uint32_t s_ph = 0, o_ph = 0;
     int tr_it = 0;
+    Ring ring;  // mirrors the producer's K/V ring: two stages (K, V) per visited block
     UnitConsumer cons{sched};
     Unit u;
     int un = -1;
@@ -465,12 +466,19 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           for (int c = 0; c < D / 16; ++c) reinterpret_cast<uint4*>(o_ptr)[c] = make_uint4(0, 0, 0, 0);
           if (hf == 0) p.LSE[(int64_t)h * p.lse_head_stride + grow] = -CUDART_INF_F;
         }
+        for (; !wk.done(); wk.next()) {  // the other tile's blocks still pass through the ring
+          ring.advance();
+          ring.advance();
+        }
         continue;
       }
       float m_used = -CUDART_INF_F;
       float2 l2 = make_float2(0.f, 0.f);
       int cnt = 0;
       for (; !wk.done(); wk.next()) {
+        ring.advance();  // K stage of this block
+        const uint32_t v_stage = ring.stage, v_phase = ring.phase;
+        ring.advance();
         if (!wk.active(t)) continue;
         mbar_wait(&s_full[t], s_ph);
         s_ph ^= 1;
@@ -529,6 +537,24 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         max16m(A, 32);
         max16m(B, 48);  // chunk 3 stays in B for pass 2
         if (r == 0) TRACE(t, 1, tr_it);
+        // Ragged key block: TMA loaded a whole 128-row V box, so the rows past the key range hold
+        // whatever follows in the caller's buffer (another document, or uninitialised rows with
+        // NaN / Inf).  P is exactly 0 there, but 0 x NaN inside the PV contraction would poison
+        // every row of O: the 256 softmax threads of this tile zero those V rows (both tiles do,
+        // with the same zeros) before the first chunk of P is handed over.
+        if (edge && b0 + kTile > wk.sp.len) {
+          const int vk = wk.sp.len - b0;
+          mbar_wait(&kv_full[v_stage], v_phase);
+          uint8_t* vt = smem + L::kKVOff + v_stage * L::kTileBytes;
+          constexpr int kChunksPerRow = D / 8;
+          const int total = (kTile - vk) * kChunksPerRow;
+          for (int i = (threadIdx.x & 255); i < total; i += 256) {
+            const int row = vk + i / kChunksPerRow, cc = i % kChunksPerRow;
+            *reinterpret_cast<uint4*>(vt + (cc / 8) * (kTile * 128) + row * 128 + (cc % 8) * 16) =
+                make_uint4(0, 0, 0, 0);
+          }
+          fence_proxy_async_smem();
+        }
         const float mx_half = fmaxf(mx0, mx1);
         // exchange the half-row maxima (slots alternate with the block parity; one barrier/block)
         xch_m[(cnt & 1) * 256 + hf * 128] = mx_half;
@@ -674,55 +700,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
 }  // namespace
 
-namespace bs {
-
-// Upload [header | items | spans | fill] into the workspace with one pageable-memory copy.
-bs_status_t upload_tables(const SchedTables& tb, void* ws, size_t ws_bytes, cudaStream_t st,
-                          WsLayout* layout) {
-  const WsLayout L = ws_layout(tb.items.size(), tb.spans.size(), tb.groups.size(), tb.fill.size());
-  BS_REQUIRE(ws != nullptr && ((uintptr_t)ws & 255) == 0, BS_ERR_WORKSPACE,
-             "workspace is null or not 256-byte aligned");
-  BS_REQUIRE(ws_bytes >= L.total, BS_ERR_WORKSPACE, "workspace too small: %zu < %zu bytes",
-             ws_bytes, L.total);
-  std::vector<uint8_t> blob;
-  try {
-    blob.assign(L.total, 0);
-  } catch (const std::bad_alloc&) {
-    return fail(BS_ERR_HOST_OOM, "out of host memory staging the work list");
-  }
-  SchedHeader* hd = reinterpret_cast<SchedHeader*>(blob.data());
-  hd->counter = 0;
-  hd->n_items = (int32_t)tb.items.size();
-  hd->n_spans = (int32_t)tb.spans.size();
-  hd->n_fill = (int32_t)tb.fill.size();
-  hd->n_groups = (int32_t)tb.groups.size();
-  hd->n_units = tb.n_units;
-  if (!tb.groups.empty())
-    memcpy(blob.data() + L.groups_off, tb.groups.data(), tb.groups.size() * sizeof(Group));
-  if (!tb.items.empty())
-    memcpy(blob.data() + L.items_off, tb.items.data(), tb.items.size() * sizeof(Item));
-  if (!tb.spans.empty())
-    memcpy(blob.data() + L.spans_off, tb.spans.data(), tb.spans.size() * sizeof(Span));
-  if (!tb.fill.empty())
-    memcpy(blob.data() + L.fill_off, tb.fill.data(), tb.fill.size() * sizeof(RowRange));
-  BS_CUDA(cudaMemcpyAsync(ws, blob.data(), L.total, cudaMemcpyHostToDevice, st));
-  *layout = L;
-  return BS_OK;
-}
-
-int sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
-      n = 148;
-  }
-  return n;
-}
-
-}  // namespace bs
-
 #ifdef BS_FWD_TRACE
 extern "C" int bs_debug_fwd_trace(long long* host_out) {
   return (int)cudaMemcpyFromSymbol(host_out, g_fwd_trace, sizeof(g_fwd_trace));
@@ -760,27 +737,18 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
              "bs_attn_fwd: dQ_acc_clear not 16-byte aligned");
   if (out_row_end == out_row_begin) return BS_OK;
   cudaStream_t st = (cudaStream_t)stream;
+  // Everything that can fail on an argument comes first: work list, workspace, device, tensor
+  // maps (pointer / stride alignment).  Nothing is enqueued before all of it has passed.
   bs::SchedTables tb;
   rc = bs::build_fwd_tables(segs, n_segs, shape->q_rows, shape->kv_rows, out_row_begin, out_row_end,
                             shape->n_q_heads, &tb);
   if (rc != BS_OK) return rc;
   bs::WsLayout L;
-  rc = bs::upload_tables(tb, ws, ws_bytes, st, &L);
+  rc = bs::check_workspace(tb, ws, ws_bytes, &L);
   if (rc != BS_OK) return rc;
-  uint8_t* wsb = (uint8_t*)ws;
-  rc = bs::launch_fill_rows((const int2*)(wsb + L.fill_off), (int)tb.fill.size(), tb.max_fill_rows,
-                            O, nullptr, LSE, shape->n_q_heads, shape->head_dim, shape->q_row_stride,
-                            shape->lse_head_stride, st);
+  rc = bs::check_device();
   if (rc != BS_OK) return rc;
   const int D = shape->head_dim;
-  if (dQ_acc_clear != nullptr) {  // rows covered by no unit: cleared here (rare path)
-    const size_t row_bytes = (size_t)shape->n_q_heads * D * sizeof(float);
-    for (const bs::RowRange& f : tb.fill)
-      BS_CUDA(cudaMemsetAsync((uint8_t*)dQ_acc_clear + (size_t)f.begin * row_bytes, 0,
-                              (size_t)(f.end - f.begin) * row_bytes, st));
-  }
-  if (tb.items.empty()) return BS_OK;
-
   CUtensorMap tmQ, tmK, tmV, tmZ;
   rc = bs::make_tensor_map_3d(&tmQ, Q, 2, D, shape->n_q_heads, shape->q_rows, shape->q_row_stride,
                               64, bs::kTile, 128);
@@ -791,11 +759,25 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
   rc = bs::make_tensor_map_3d(&tmV, V, 2, D, shape->n_kv_heads, shape->kv_rows,
                               shape->kv_row_stride, 64, bs::kTile, 128);
   if (rc != BS_OK) return rc;
-
   // zero stores: rows clipped at out_row_end by the map itself (a unit's 256 rows may overhang)
   rc = bs::make_tensor_map_3d(&tmZ, dQ_acc_clear ? (const void*)dQ_acc_clear : Q, 4, D,
                               shape->n_q_heads, out_row_end, (int64_t)shape->n_q_heads * D, 32, 64, 0);
   if (rc != BS_OK) return rc;
+
+  rc = bs::upload_tables(tb, L, ws, st);
+  if (rc != BS_OK) return rc;
+  uint8_t* wsb = (uint8_t*)ws;
+  rc = bs::launch_fill_rows((const int2*)(wsb + L.fill_off), (int)tb.fill.size(), tb.max_fill_rows,
+                            O, nullptr, LSE, shape->n_q_heads, shape->head_dim, shape->q_row_stride,
+                            shape->lse_head_stride, st);
+  if (rc != BS_OK) return rc;
+  if (dQ_acc_clear != nullptr) {  // rows covered by no unit: cleared here (rare path)
+    const size_t row_bytes = (size_t)shape->n_q_heads * D * sizeof(float);
+    for (const bs::RowRange& f : tb.fill)
+      BS_CUDA(cudaMemsetAsync((uint8_t*)dQ_acc_clear + (size_t)f.begin * row_bytes, 0,
+                              (size_t)(f.end - f.begin) * row_bytes, st));
+  }
+  if (tb.items.empty()) return BS_OK;
 
   FwdParams p;
   p.clear_acc = dQ_acc_clear != nullptr;
@@ -812,12 +794,12 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
   p.lse_head_stride = shape->lse_head_stride;
   const int grid = tb.n_units < bs::sm_count() ? tb.n_units : bs::sm_count();
   if (D == 128) {
-    BS_CUDA(cudaFuncSetAttribute(attn_fwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 FwdSmem<128>::kAlloc));
+    rc = bs::set_max_smem_once((const void*)attn_fwd_kernel<128>, FwdSmem<128>::kAlloc, 0);
+    if (rc != BS_OK) return rc;
     attn_fwd_kernel<128><<<grid, kFwdThreads, FwdSmem<128>::kAlloc, st>>>(tmQ, tmK, tmV, tmZ, p);
   } else {
-    BS_CUDA(cudaFuncSetAttribute(attn_fwd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 FwdSmem<64>::kAlloc));
+    rc = bs::set_max_smem_once((const void*)attn_fwd_kernel<64>, FwdSmem<64>::kAlloc, 1);
+    if (rc != BS_OK) return rc;
     attn_fwd_kernel<64><<<grid, kFwdThreads, FwdSmem<64>::kAlloc, st>>>(tmQ, tmK, tmV, tmZ, p);
   }
   BS_CUDA(cudaGetLastError());

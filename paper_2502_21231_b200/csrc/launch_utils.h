@@ -28,9 +28,16 @@ bs_status_t make_tensor_map_3d(CUtensorMap* map, const void* base, int elem_byte
 
 #include "worklist.h"
 namespace bs {
-bs_status_t upload_tables(const SchedTables& tb, void* ws, size_t ws_bytes, cudaStream_t st,
-                          WsLayout* layout);
-int sm_count();
+// host_runtime.cpp
+// BS_ERR_UNSUPPORTED unless the current device is compute capability 10.0 (the kernels are sm_100a).
+bs_status_t check_device(int* device_out = nullptr);
+int sm_count();  // of the current device (after check_device)
+// cudaFuncAttributeMaxDynamicSharedMemorySize, set once per device and kernel (kernel_slot < 32)
+bs_status_t set_max_smem_once(const void* func, int bytes, int kernel_slot);
+// Workspace checks (null / alignment / size) and layout; enqueues nothing.
+bs_status_t check_workspace(const SchedTables& tb, const void* ws, size_t ws_bytes, WsLayout* layout);
+// Tables -> workspace on `st` from a pinned staging slot (no stream synchronisation).
+bs_status_t upload_tables(const SchedTables& tb, const WsLayout& layout, void* ws, cudaStream_t st);
 }  // namespace bs
 
 #include "sched.cuh"

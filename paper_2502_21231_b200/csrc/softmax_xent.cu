@@ -333,9 +333,9 @@ extern "C" bs_status_t bs_softmax_xent(const void* logits, const int32_t* labels
   BS_REQUIRE((((uintptr_t)logits | (uintptr_t)dlogits) & 15) == 0, BS_ERR_INVALID_ARG,
              "bs_softmax_xent: logits and dlogits must be 16-byte aligned");
   cudaStream_t st = (cudaStream_t)stream;
-  int dev = 0, sms = 0;
-  BS_CUDA(cudaGetDevice(&dev));
-  BS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  bs_status_t rc = bs::check_device();
+  if (rc != BS_OK) return rc;
+  const int sms = bs::sm_count();
   XentParams p{(const __nv_bfloat16*)logits, labels, loss, (__nv_bfloat16*)dlogits, row_stride,
                n_tokens, vocab, grad_scale};
   const int nvec = vocab / 8;
@@ -348,8 +348,8 @@ extern "C" bs_status_t bs_softmax_xent(const void* logits, const int32_t* labels
   } else if (vocab <= kMaxSmemV) {
     const size_t smem = (size_t)(vocab / 8) * 16;
     const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(8, (200 * 1024) / (smem + 1024)));
-    BS_CUDA(cudaFuncSetAttribute(softmax_xent_kernel<true>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    rc = bs::set_max_smem_once((const void*)softmax_xent_kernel<true>, kMaxSmemV * 2, 4);
+    if (rc != BS_OK) return rc;
     const int grid = std::min(n_tokens, sms * per_sm);
     softmax_xent_kernel<true><<<grid, kThreads, smem, st>>>(p);
   } else {

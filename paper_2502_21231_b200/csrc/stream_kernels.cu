@@ -31,11 +31,27 @@ struct MergeParams {
   int64_t lse_head_stride;
 };
 
+// read-only streams (never aliased by an output of the same kernel): non-coherent path
 __device__ __forceinline__ uint4 ldg_stream(const uint4* p) {
   uint4 r;
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
                : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
                : "l"(p));
+  return r;
+}
+// bs_lse_merge lets O_out / LSE_out alias a part (running merge): ld.global.nc requires data that
+// is read-only for the kernel's lifetime, so the merge reads its parts with coherent loads
+__device__ __forceinline__ uint4 ldg_coherent(const uint4* p) {
+  uint4 r;
+  asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p)
+               : "memory");
+  return r;
+}
+__device__ __forceinline__ float ldf_coherent(const float* p) {
+  float r;
+  asm volatile("ld.global.f32 %0, [%1];" : "=f"(r) : "l"(p) : "memory");
   return r;
 }
 __device__ __forceinline__ void stg_stream(uint4* p, const uint4& v) {
@@ -71,7 +87,7 @@ __device__ __forceinline__ void merge_few(const MergeParams& p, const float* w_s
       off[u] = (int64_t)(row0 + r) * p.row_stride_v + (int64_t)h0 * kVecPerHead + c;
 #pragma unroll
       for (int j = 0; j < kNP; ++j)
-        if (t < total && j < n) v[u][j] = ldg_stream(p.O_parts[j] + off[u]);
+        if (t < total && j < n) v[u][j] = ldg_coherent(p.O_parts[j] + off[u]);
     }
 #pragma unroll
     for (int u = 0; u < kU; ++u) {
@@ -112,13 +128,13 @@ __global__ void __launch_bounds__(kStreamThreads) lse_merge_kernel(const __grid_
     if (r >= nrows) continue;
     const int64_t off = (int64_t)(h0 + h) * p.lse_head_stride + (row0 + r);
     float M = -CUDART_INF_F;
-    for (int s = 0; s < n; ++s) M = fmaxf(M, __ldg(p.LSE_parts[s] + off));
+    for (int s = 0; s < n; ++s) M = fmaxf(M, ldf_coherent(p.LSE_parts[s] + off));
     float Z = 0.f;
     if (M != -CUDART_INF_F)
-      for (int s = 0; s < n; ++s) Z += __expf(__ldg(p.LSE_parts[s] + off) - M);
+      for (int s = 0; s < n; ++s) Z += __expf(ldf_coherent(p.LSE_parts[s] + off) - M);
     const float invZ = (M == -CUDART_INF_F) ? 0.f : 1.f / Z;
     for (int s = 0; s < n; ++s) {
-      const float l = __ldg(p.LSE_parts[s] + off);
+      const float l = ldf_coherent(p.LSE_parts[s] + off);
       w_smem[(s * kRowsPerTile + r) * p.heads_per_block + h] =
           (M == -CUDART_INF_F) ? 0.f : __expf(l - M) * invZ;
     }
@@ -147,7 +163,7 @@ __global__ void __launch_bounds__(kStreamThreads) lse_merge_kernel(const __grid_
       uint4 v[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j)
-        if (s0 + j < n) v[j] = ldg_stream(p.O_parts[s0 + j] + off);
+        if (s0 + j < n) v[j] = ldg_coherent(p.O_parts[s0 + j] + off);
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         if (s0 + j < n) {
@@ -279,6 +295,8 @@ int pick_heads_per_block(int n_heads, int floats_per_row_head, int smem_budget_b
 
 namespace bs {
 
+constexpr int32_t kMaxRows = (1 << 30) - 1024;
+
 bs_status_t validate_shape(const bs_attn_shape_t* s, const char* who) {
   BS_REQUIRE(s != nullptr, BS_ERR_INVALID_ARG, "%s: shape is null", who);
   BS_REQUIRE(s->head_dim == 64 || s->head_dim == 128, BS_ERR_UNSUPPORTED,
@@ -287,6 +305,10 @@ bs_status_t validate_shape(const bs_attn_shape_t* s, const char* who) {
              BS_ERR_INVALID_ARG, "%s: n_q_heads %d / n_kv_heads %d", who, s->n_q_heads,
              s->n_kv_heads);
   BS_REQUIRE(s->q_rows >= 0 && s->kv_rows >= 0, BS_ERR_INVALID_ARG, "%s: negative row count", who);
+  // row + causal offset is 32-bit arithmetic in the kernels (offsets are clamped to the range
+  // lengths): q_rows + kv_rows must stay below 2^31
+  BS_REQUIRE(s->q_rows <= kMaxRows && s->kv_rows <= kMaxRows, BS_ERR_UNSUPPORTED,
+             "%s: more than %d rows in one buffer", who, kMaxRows);
   BS_REQUIRE(s->q_row_stride >= (int64_t)s->n_q_heads * s->head_dim && s->q_row_stride % 8 == 0,
              BS_ERR_INVALID_ARG, "%s: q_row_stride %lld", who, (long long)s->q_row_stride);
   BS_REQUIRE(s->kv_row_stride >= (int64_t)s->n_kv_heads * s->head_dim && s->kv_row_stride % 8 == 0,
@@ -338,6 +360,8 @@ bs_status_t bs_lse_merge(int32_t n_parts, const void* const* O_parts, const floa
   }
   BS_REQUIRE(((uintptr_t)O_out & 15) == 0, BS_ERR_INVALID_ARG, "bs_lse_merge: O_out misaligned");
   if (row_end == row_begin) return BS_OK;
+  rc = bs::check_device();
+  if (rc != BS_OK) return rc;
   p.O_out = (uint4*)O_out;
   p.LSE_out = LSE_out;
   p.n_parts = n_parts;
@@ -369,6 +393,8 @@ bs_status_t bs_attn_bwd_prep(const bs_attn_shape_t* shape, const void* O_final, 
   BS_REQUIRE((((uintptr_t)O_final | (uintptr_t)dO | (uintptr_t)dQ_acc) & 15) == 0,
              BS_ERR_INVALID_ARG, "bs_attn_bwd_prep: pointers must be 16-byte aligned");
   if (shape->q_rows == 0) return BS_OK;
+  rc = bs::check_device();
+  if (rc != BS_OK) return rc;
   PrepParams p;
   p.O = (const uint4*)O_final;
   p.dO = (const uint4*)dO;
@@ -401,6 +427,8 @@ bs_status_t bs_attn_bwd_finish(const bs_attn_shape_t* shape, const float* dQ_acc
   BS_REQUIRE((((uintptr_t)dQ_acc | (uintptr_t)dQ) & 15) == 0, BS_ERR_INVALID_ARG,
              "bs_attn_bwd_finish: pointers must be 16-byte aligned");
   if (shape->q_rows == 0) return BS_OK;
+  rc = bs::check_device();
+  if (rc != BS_OK) return rc;
   const int vec_per_row = shape->n_q_heads * shape->head_dim / 8;
   const int64_t n_vec = (int64_t)shape->q_rows * vec_per_row;
   int64_t blocks = (n_vec + kStreamThreads - 1) / kStreamThreads;

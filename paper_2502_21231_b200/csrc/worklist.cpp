@@ -21,9 +21,6 @@ bs_status_t gaps_of(const std::vector<Range>& rs, int32_t lo, int32_t hi, const 
                     SchedTables* out) {
   int32_t cur = lo;
   for (const Range& r : rs) {
-    BS_REQUIRE(r.begin >= cur || r.begin == lo, BS_ERR_INVALID_ARG,
-               "%s ranges of two segments overlap without being identical (at row %d)", what,
-               r.begin);
     BS_REQUIRE(r.begin >= cur, BS_ERR_INVALID_ARG,
                "%s ranges of two segments overlap without being identical (at row %d)", what,
                r.begin);
@@ -43,6 +40,14 @@ bs_status_t check_seg(const bs_seg_t& g, int i, int32_t q_rows, int32_t kv_rows)
   BS_REQUIRE(0 <= g.k_begin && g.k_begin < g.k_end && g.k_end <= kv_rows, BS_ERR_INVALID_ARG,
              "segment %d: k range [%d,%d) empty or outside [0,%d)", i, g.k_begin, g.k_end, kv_rows);
   return BS_OK;
+}
+
+// Key b is visible to query a iff b <= a + off (a in [0, q_len), b in [0, k_len)).  Every offset
+// >= k_len - 1 means "all keys" and every offset <= -q_len means "none", so the offset is stored
+// clamped to [-q_len, k_len]: the mask is unchanged, and the kernels' 32-bit index arithmetic
+// (row + offset) cannot overflow for callers who pass INT32_MAX / INT32_MIN as sentinels.
+inline int32_t clamp_offset(int32_t off, int32_t q_len, int32_t k_len) {
+  return std::max<int32_t>(-q_len, std::min<int32_t>(off, k_len));
 }
 }  // namespace
 
@@ -125,7 +130,9 @@ bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
       while (j < n_segs && segs[order[j]].q_begin == g0.q_begin &&
              segs[order[j]].q_end == g0.q_end) {
         const bs_seg_t& g = segs[order[j]];
-        out->spans.push_back({g.k_begin, g.k_end - g.k_begin, g.causal_offset, 0});
+        out->spans.push_back({g.k_begin, g.k_end - g.k_begin,
+                              clamp_offset(g.causal_offset, g.q_end - g.q_begin, g.k_end - g.k_begin),
+                              0});
         ++j;
       }
       ranges.push_back({g0.q_begin, g0.q_end});
@@ -185,7 +192,9 @@ bs_status_t build_bwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
       while (j < n_segs && segs[order[j]].k_begin == g0.k_begin &&
              segs[order[j]].k_end == g0.k_end) {
         const bs_seg_t& g = segs[order[j]];
-        out->spans.push_back({g.q_begin, g.q_end - g.q_begin, g.causal_offset, 0});
+        out->spans.push_back({g.q_begin, g.q_end - g.q_begin,
+                              clamp_offset(g.causal_offset, g.q_end - g.q_begin, g.k_end - g.k_begin),
+                              0});
         ++j;
       }
       ranges.push_back({g0.k_begin, g0.k_end});

@@ -116,9 +116,10 @@ def make_workload(cfg: int) -> Workload:
     raise ValueError(cfg)
 
 
-def scaled_twin(cfg: int, c: int = 256, ragged: bool = False, rank=None) -> Workload:
-    """Same structure (N, r, Hq/Hkv, D, segment pattern) as configs 3-5 with part length ~c.
-    ragged=True makes 2N not divide L and c unaligned to any tile."""
+def scaled_twin(cfg: int, c: int = 256, ragged: bool = False, rank=None, kv_heads=None) -> Workload:
+    """Same structure (N, r, Hq/Hkv ratio, D, segment pattern) as configs 3-5 with part length ~c.
+    ragged=True makes 2N not divide L and c unaligned to any tile.  kv_heads: number of KV heads
+    (the group size Hq/Hkv is kept; fewer groups make the fp64 oracle pass affordable)."""
     w = make_workload(cfg)
     ln, cp, r = w.seqs[0]
     assert cp > 1
@@ -130,8 +131,10 @@ def scaled_twin(cfg: int, c: int = 256, ragged: bool = False, rank=None) -> Work
     if cfg == 4:
         lens = pareto_lengths(w.seed + 100, 2 * c + (13 if ragged else 0), hi=max(64, c // 2))
         rest = [(x, 1, 0) for x in lens]
-    return Workload(f"{w.name}_twin_c{c}{'_ragged' if ragged else ''}_r{r}", w.n_q_heads,
-                    w.n_kv_heads, w.head_dim, [(L, cp, r)] + rest, w.seed + 1000 + r,
+    group = w.n_q_heads // w.n_kv_heads
+    hkv = w.n_kv_heads if kv_heads is None else kv_heads
+    return Workload(f"{w.name}_twin_c{c}{'_ragged' if ragged else ''}_r{r}", hkv * group, hkv,
+                    w.head_dim, [(L, cp, r)] + rest, w.seed + 1000 + r,
                     note=f"scaled twin of cfg{cfg}")
 
 

@@ -160,27 +160,118 @@ class DeviceRun:
         return dQ, out
 
 
-def check_forward(run, O, LSE, rows=None):
+def o_compare(got_O, Oo, label=""):
+    """O against the oracle, element by element.  BASELINE.json's bound is 1.5e-2 max-abs.  A bf16
+    output cannot meet it where the output FORMAT alone is off by more: half an ulp is 1.5625e-2
+    for |O| in [4, 8).  DESIGN.md reading 19: the strict bound holds for every element except
+    those whose own quantisation floor |bf16(O_oracle) - O_oracle| exceeds 1.5e-2 - 4e-3; those
+    are bounded by their floor + 4e-3.  Prints how many elements that concerns, the largest error
+    among the strictly bounded ones and the floor, and asserts.  Returns the max abs error."""
+    diff = np.abs(got_O - Oo)
+    floor = np.abs(bf16_round(Oo) - Oo)
+    loose = floor > TOL_O - 4e-3
+    tol = np.where(loose, floor + 4e-3, TOL_O)
+    n_big = int((np.abs(Oo) >= 4.0).sum())
+    strict_max = float(diff[~loose].max()) if (~loose).any() else 0.0
+    print(f"{label}O: {diff.size} elements, max abs err {float(diff.max()):.3e} (strict bound "
+          f"{TOL_O}: max {strict_max:.3e} over {int((~loose).sum())} elements); |O| >= 4: {n_big} "
+          f"elements; bf16 quantisation floor of the oracle values: max {float(floor.max()):.3e}, "
+          f"{int(loose.sum())} elements above {TOL_O - 4e-3:.1e} (bounded by floor + 4e-3)")
+    assert np.all(diff <= tol), (f"{label}O max abs err {float(diff.max())}; worst excess over the "
+                                 f"per-element bound {float((diff - tol).max())}")
+    return float(diff.max())
+
+
+def grad_compare(name, got, want, block_of_row, label=""):
+    """One gradient tensor [rows, heads, D] against the oracle: relative L2 over the whole tensor
+    AND over every (document, head) block (a broken short document cannot hide behind a long
+    one), plus an element-wise bound.  Tolerance: BASELINE.json's 1e-2 relative L2, applied to
+    the whole tensor and to each block; a block whose oracle gradient is identically zero (a
+    length-1 document's dQ / dK) must be zero to 1e-4 rms.  Element-wise: the kernels round P and
+    dS to bf16 before the second MMAs, so an element's error is a random walk of relative steps
+    2^-9 over terms whose root-sum-square is of the order of the block's rms, plus the final bf16
+    rounding: |err| <= 2^-8 |want| + 0.06 rms(block)."""
+    got = np.asarray(got, np.float64)
+    want = np.asarray(want, np.float64)
+    assert got.shape == want.shape and got.ndim == 3
+    assert not np.isnan(got).any(), f"{label}{name} has NaN"
+    whole = rel_l2(got, want)
+    blk = np.asarray(block_of_row, np.int64)
+    nb = int(blk.max()) + 1 if len(blk) else 0
+    H, D = got.shape[1], got.shape[2]
+    num = np.zeros((nb, H))
+    den = np.zeros((nb, H))
+    cnt = np.bincount(blk, minlength=nb).astype(np.float64)[:, None] * D
+    np.add.at(num, blk, ((got - want) ** 2).sum(-1))
+    np.add.at(den, blk, (want ** 2).sum(-1))
+    live = cnt[:, 0] > 0
+    zero = (den == 0) & live[:, None]
+    rel = np.sqrt(num / np.where(den > 0, den, 1.0))
+    rel[~(den > 0)] = 0.0
+    worst = float(rel.max()) if rel.size else 0.0
+    zero_rms = float(np.sqrt((num / np.maximum(cnt, 1))[zero]).max()) if zero.any() else 0.0
+    rms = np.sqrt(den / np.maximum(cnt, 1))                     # [blocks, heads]
+    bound = 2.0 ** -8 * np.abs(want) + 0.06 * rms[blk][:, :, None] + 1e-6
+    ratio = float((np.abs(got - want) / bound).max()) if got.size else 0.0
+    print(f"{label}{name}: rel-L2 whole {whole:.2e}, worst (document, head) block {worst:.2e} over "
+          f"{int(live.sum())} x {H} blocks, zero-gradient blocks rms {zero_rms:.1e}, "
+          f"element-wise err / bound max {ratio:.2f}")
+    assert whole <= TOL_GRAD, f"{label}{name} relative L2 error {whole}"
+    assert worst <= TOL_GRAD, (f"{label}{name} relative L2 error {worst} in (document, head) block "
+                               f"{np.unravel_index(int(rel.argmax()), rel.shape)}")
+    assert zero_rms <= 1e-4, f"{label}{name}: block with zero oracle gradient has rms {zero_rms}"
+    assert ratio <= 1.0, f"{label}{name}: element-wise error {ratio} x the bound"
+    return whole
+
+
+def check_forward(run, O, LSE, rows=None, label=""):
     Oo, Lo = run.oracle_forward(rows)
     got_O = oracle.bf16_to_f64(to_bits(O)).reshape(run.q_rows, run.Hq, run.D)
     got_L = LSE.double().cpu().numpy()
     if rows is not None:
         got_O, got_L = got_O[rows], got_L[:, rows]
     assert not np.isnan(got_O).any() and not np.isnan(got_L).any()
-    # O tolerance (reading 19): BASELINE.json's 1.5e-2 max-abs wherever a bf16 output can
-    # meet it, i.e. |O| < 4 (half-ulp <= 7.8e-3).  For |O| >= 4 the output FORMAT alone can be off by
-    # half an ulp = 2^(e-8) >= 1.5625e-2 (a tie in the oracle value rounds either way), so the bound
-    # there is that half-ulp plus the 4e-3 of arithmetic slack that 1.5e-2 leaves below |O| < 4.
-    diff = np.abs(got_O - Oo)
-    half_ulp = 2.0 ** (np.floor(np.log2(np.maximum(np.abs(Oo), 1e-30))) - 8)
-    tol = np.where(np.abs(Oo) < 4.0, TOL_O, half_ulp + 4e-3)
-    err_O = float(diff.max())
-    floor = float(np.abs(bf16_round(Oo) - Oo).max())
-    assert np.all(diff <= tol), (f"O max abs err {err_O} (bf16 quantisation floor of the oracle "
-                                 f"values {floor}); worst excess {float((diff - tol).max())}")
+    err_O = o_compare(got_O, Oo, label)
     fin = np.isfinite(Lo)
     assert np.array_equal(np.isneginf(got_L), np.isneginf(Lo))
     err_L = float(np.abs(got_L[fin] - Lo[fin]).max()) if fin.any() else 0.0
     assert np.all(got_O[~fin.T] == 0)
-    assert err_L <= TOL_LSE, f"LSE abs err {err_L}"
+    assert err_L <= TOL_LSE, f"{label}LSE abs err {err_L}"
     return err_O, err_L
+
+
+def _blocks(step_idx, seq, n_seq):
+    """Block id per row: (step, document, 128-row chunk of the document's rows in the buffer)."""
+    seq = np.asarray(seq, np.int64)
+    n = len(seq)
+    start = np.zeros(n, np.int64)  # index of the first row of each run of equal seq
+    if n:
+        brk = np.flatnonzero(seq[1:] != seq[:-1]) + 1
+        first = np.concatenate(([0], brk))
+        start = np.repeat(first, np.diff(np.concatenate((first, [n]))))
+    chunk = (np.arange(n) - start) // 128
+    key = (step_idx * n_seq + seq) * (n // 128 + 2) + chunk
+    _, ids = np.unique(key, return_inverse=True)
+    return ids
+
+
+def check_backward(run, dQ, grads, label=""):
+    """dQ, dK, dV of a DeviceRun against the oracle over all keys: whole tensor, every block of
+    (ring step, document, 128 buffer rows) x head, and element-wise (grad_compare).  Returns the
+    whole-tensor errors."""
+    dQo, go = run.oracle_backward()
+    opl = oracle.oracle_plan(run.w.seqs)
+    n_seq = len(run.w.seqs)
+    got = oracle.bf16_to_f64(to_bits(dQ)).reshape(dQo.shape)
+    errs = {"dQ": grad_compare("dQ", got, dQo, _blocks(0, opl["q_seq"], n_seq), label)}
+    kblk, base = [], 0
+    for s in run.steps:
+        b = _blocks(0, opl["steps"][s]["k_seq"], n_seq) + base
+        base = int(b.max()) + 1 if len(b) else base
+        kblk.append(b)
+    kblk = np.concatenate(kblk)
+    for i, n in ((0, "dK"), (1, "dV")):
+        g = np.concatenate([oracle.bf16_to_f64(to_bits(grads[s][i])).reshape(go[s][i].shape)
+                            for s in run.steps])
+        errs[n] = grad_compare(n, g, np.concatenate([go[s][i] for s in run.steps]), kblk, label)
+    return errs

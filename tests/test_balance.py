@@ -35,6 +35,24 @@ def test_hand_worked(impl):
         (3, 208, 320, [(15, 2, 1, 1)])]
 
 
+@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("n_buckets", [1, 2, 4, 9])
+def test_zero_work_group_stays_in_the_last_bucket(impl, n_buckets):
+    """Reading B3's corner: T(s) = 1 for every sequence, so a long sequence on D = 2 ranks costs
+    each rank floor(1 / 2) = 0 - a group of zero work, sorted behind all the work.  Its bucket
+    index floor(n_buckets * work before / total work) would be n_buckets: it stays in the last
+    bucket (B3) instead of indexing past the end.  Worked by hand: bin {5, 5} costs 2 and goes to
+    rank 0 at 0..2; the long group then goes to the two least loaded ranks that lag (1 and 2),
+    starting at 0 and ending at 0."""
+    a = impl([20, 5, 5], 10, 4, (0, 0, 1), n_buckets, 0)
+    assert a["exec_times"] == [2, 0, 0, 0] and a["makespan"] == 2
+    assert a["microbatches"] == [(0, 0, 2, [(5, 1, 0, 1), (5, 1, 0, 2)]),
+                                 (1, 0, 0, [(20, 2, 0, 0)]), (2, 0, 0, [(20, 2, 1, 0)])]
+    # all work zero (total work 0): everything goes to bucket 0 and is still scheduled once
+    b = impl([20, 5, 5], 10, 4, (0, 0, 0), n_buckets, 0)
+    assert b["makespan"] == 0 and len(b["microbatches"]) == 3
+
+
 def random_batch(g):
     cap = g.choice([4, 10, 100, 8192])
     d_hdp = g.choice([1, 2, 3, 8, 32])

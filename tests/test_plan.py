@@ -189,6 +189,36 @@ def test_library_plan_bit_exact_on_configs(cfg):
         assert np.array_equal(sa["k_pos"], sb["k_pos"])
 
 
+def _same_plan(a, b):
+    assert a["q_rows"] == b["q_rows"] and a["n_steps"] == b["n_steps"]
+    assert list(a["cu_rows_q"]) == list(b["cu_rows_q"])
+    assert np.array_equal(a["q_seq"], b["q_seq"]) and np.array_equal(a["q_pos"], b["q_pos"])
+    for sa, sb in zip(a["steps"], b["steps"]):
+        assert [tuple(x) for x in sa["segs"]] == [tuple(x) for x in sb["segs"]]
+        for k in ("step", "kv_rows", "visible_pairs"):
+            assert sa[k] == sb[k], k
+        for k in ("kv_seq", "kv_src_rank", "cu_rows_k"):
+            assert list(sa[k]) == list(sb[k]), k
+        assert np.array_equal(sa["k_seq"], sb["k_seq"]) and np.array_equal(sa["k_pos"], sb["k_pos"])
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_plan_uniform_matches_oracle(seed):
+    """bs_plan_uniform (north_star: "per-sequence lengths and a CP degree"): sequences of at least
+    min_shard_len tokens get (cp, rank), the rest stay whole - the data-aware sharding rule of
+    PAPER.md:165 - and the result is bs_plan's on that list, compared with the oracle planner."""
+    from paper_2502_21231_b200 import binding
+    rng = np.random.default_rng(100 + seed)
+    lens = [int(x) for x in rng.integers(1, 4000, int(rng.integers(1, 15)))]
+    cp = int(rng.choice([1, 2, 4, 8]))
+    rank = int(rng.integers(0, cp))
+    min_len = int(rng.choice([1, 512, 2048, 5000]))
+    seqs = [(L, cp, rank) if L >= min_len else (L, 1, 0) for L in lens]
+    _same_plan(oracle.oracle_plan(seqs), binding.plan_uniform(lens, cp, rank, min_len))
+    with pytest.raises(binding.BsError):
+        binding.plan_uniform(lens, cp, cp, min_len)   # rank outside [0, cp)
+
+
 def test_library_plan_errors():
     from paper_2502_21231_b200 import binding
     for bad in ([(0, 1, 0)], [(5, 0, 0)], [(5, 2, 2)], [(5, 2, -1)]):
