@@ -13,6 +13,10 @@ N > 1: every rank runs its own cfg2-shaped batch (weak scaling, no data-path col
 HDP ranks are independent per micro-batch); torch.distributed is used only for
 the barrier and the max-over-ranks of the device time.
 --impl reference: times the fp64 oracle (the reference arm of this tier) on the host cores.
+--gpus N with N > 1 and no WORLD_SIZE in the environment: bench.py starts the N ranks itself
+(python -m torch.distributed.run, one process per GPU, rendezvous on 127.0.0.1).
+--impl plumbing: the launch path alone on CPU (gloo): every rank times a host-only step (bs_plan),
+barrier, max over ranks, rank 0 prints the line - what tests/test_dist_gloo.py drives with 2 ranks.
 """
 import argparse
 import json
@@ -43,14 +47,19 @@ def peaks():
 
 
 def ncu_traffic(kernel_prefix):
-    """DRAM bytes (read + write) per launch of a kernel from the committed ncu capture
-    (profiles/r01_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum of one
-    `ncu --set full` launch on this workload), or None."""
-    path = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    """DRAM bytes (read + write) per launch of a kernel from this round's ncu capture
+    (profiles/r02_traffic.csv: kernel, dram__bytes_read.sum, dram__bytes_write.sum, sha256[:16] of
+    the kernel's source file at capture time), or None.  It cannot be measured inside this run
+    (no profiler here); a capture of OTHER source than the one that is running is not reported."""
+    import hashlib
+    path = os.path.join(ROOT, "profiles", "r02_traffic.csv")
     try:
         for line in open(path).read().splitlines()[1:]:
             f = line.split(",")
             if f[0].startswith(kernel_prefix):
+                src = os.path.join(ROOT, "paper_2502_21231_b200", "csrc", f[3])
+                if hashlib.sha256(open(src, "rb").read()).hexdigest()[:16] != f[4].strip():
+                    return None
                 return int(f[1]) + int(f[2])
     except (OSError, ValueError, IndexError):
         pass
@@ -63,7 +72,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index):
         super().__init__(daemon=True)
         self.index, self.samples, self.reasons, self.stop_flag = index, [], set(), False
-        self.max_mhz = None
+        self.stamps, self.max_mhz = [], None
 
     def run(self):
         try:
@@ -77,6 +86,7 @@ class ClockSampler(threading.Thread):
                      nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
             while not self.stop_flag:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                self.stamps.append(time.perf_counter())
                 r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
                 for bit, name in names.items():
                     if r & bit:
@@ -84,6 +94,10 @@ class ClockSampler(threading.Thread):
                 time.sleep(0.02)
         except Exception as e:  # NVML missing: report nothing rather than fail the bench
             self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def median_between(self, t0, t1):
+        s = sorted(v for v, t in zip(self.samples, self.stamps) if t0 <= t <= t1)
+        return s[len(s) // 2] if s else None
 
     def result(self):
         s = sorted(self.samples)
@@ -192,6 +206,8 @@ def run_ours(args, rank, world, local_rank):
         if marks:
             marks[3].record()
         B.attn_bwd_finish(sh, acc, dQ)
+        if marks:
+            marks[4].record()
 
     def barrier():
         torch.cuda.synchronize()
@@ -204,7 +220,7 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    marks = [[ev() for _ in range(4)] for _ in range(args.steps)]
+    marks = [[ev() for _ in range(5)] for _ in range(args.steps)]
     B.launch_count_reset()
     e0, e1 = ev(), ev()
     e0.record()
@@ -215,7 +231,37 @@ def run_ours(args, rank, world, local_rank):
     launches = B.launch_count()
     ms = e0.elapsed_time(e1)
     t_fwd = sum(m[0].elapsed_time(m[1]) for m in marks) / args.steps
+    t_prep = sum(m[1].elapsed_time(m[2]) for m in marks) / args.steps
     t_bwd = sum(m[2].elapsed_time(m[3]) for m in marks) / args.steps
+    t_fin = sum(m[3].elapsed_time(m[4]) for m in marks) / args.steps
+    if args.only_step:
+        sampler.stop_flag = True
+        sampler.join()
+        (ms,) = DU.max_over_ranks(dist, [ms], "cuda")
+        if rank == 0:
+            fl = 14.0 * D * Hq * pairs
+            print(json.dumps({"metric": METRIC, "value": world * fl * args.steps / (ms * 1e-3) / 1e12,
+                              "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
+                              "ms_per_step": ms / args.steps, "only_step": True,
+                              "kernels_ms": {"bs_attn_fwd": t_fwd, "bs_attn_bwd_prep": t_prep,
+                                             "bs_attn_bwd": t_bwd, "bs_attn_bwd_finish": t_fin},
+                              "gpu_launches": launches, "clocks": sampler.result()}))
+        if dist:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+    # sustained leg (north_star: "sustains"): the same step back to back for >= 2 s, so that the
+    # part sits at its power cap; reported against the measured SUSTAINED bf16 peak
+    n_sus = max(args.steps, int(2200.0 / (ms / args.steps)))
+    s0, s1 = ev(), ev()
+    t_sus0 = time.perf_counter()
+    s0.record()
+    for _ in range(n_sus):
+        step()
+    s1.record()
+    barrier()
+    t_sus1 = time.perf_counter()
+    ms_sus = s0.elapsed_time(s1)
     # end to end: every step copies its inputs from pinned host memory, runs, and copies its results
     # back, all inside the timed region.  The copies are PCIe-bound (1 GiB each way per step), so the
     # steps are software-pipelined over three streams with two sets of device buffers: while step i
@@ -272,7 +318,7 @@ def run_ours(args, rank, world, local_rank):
     ms_e2e = f0.elapsed_time(f1)
     sampler.stop_flag = True
     sampler.join()
-    ms, ms_e2e = DU.max_over_ranks(dist, [ms, ms_e2e], "cuda")
+    ms, ms_e2e, ms_sus = DU.max_over_ranks(dist, [ms, ms_e2e, ms_sus], "cuda")
     flops_step = 14.0 * D * Hq * pairs
     out = None
     if rank == 0:
@@ -298,32 +344,54 @@ def run_ours(args, rank, world, local_rank):
                            f"d_hdp {HDP_RANKS}, {Hq} heads, D {D}")
         dt, fl, thr = oracle_sample_run(w, CPU_BASELINE_HEADS)
         bwd_tflops = 10.0 * D * Hq * pairs / (t_bwd * 1e-3) / 1e12
+        fwd_tflops = 4.0 * D * Hq * pairs / (t_fwd * 1e-3) / 1e12
+        value = world * flops_step * args.steps / (ms * 1e-3) / 1e12
+        sus = world * flops_step * n_sus / (ms_sus * 1e-3) / 1e12
+        prep_bytes = rows * Hq * (4 * D + 4)          # reads O, dO; writes delta (dQ_acc cleared by fwd)
+        fin_bytes = rows * Hq * 6 * D                 # reads fp32 dQ_acc, writes bf16 dQ
+        # The driver keeps the contract keys of this line and the END of stdout: the long replay
+        # records come first, what explains the headline (kernels, sustained, merge) sits inside
+        # "roofline" and at the end.
         out = {
-            "metric": METRIC, "value": world * flops_step * args.steps / (ms * 1e-3) / 1e12,
+            "metric": METRIC, "value": value,
             "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": WORKLOAD, "tokens": rows, "documents": len(w.seqs),
                        "n_q_heads": Hq, "n_kv_heads": Hkv, "head_dim": D,
                        "visible_pairs_per_head": pairs, "flops_per_step": flops_step,
+                       "computed_over_visible": tile_area_ratio(w),
                        "l2": "inputs+outputs 2.4 GB per step exceed the 126 MB L2; no flush",
                        "peaks": pk["source"]},
-            "pct_of_bf16_peak": {"measured_burst": 100 * flops_step * args.steps / (ms * 1e-3) / 1e12 / pk["tflops"],
-                                 "nominal_2250": 100 * flops_step * args.steps / (ms * 1e-3) / 1e12 / 2250.0},
-            "kernels_ms": {"bs_attn_fwd": t_fwd, "bs_attn_bwd": t_bwd,
-                           "fwd_tflops": 4.0 * D * Hq * pairs / (t_fwd * 1e-3) / 1e12,
-                           "bwd_tflops": bwd_tflops},
-            "roofline": {"kernel": "attn_bwd_kernel<128>", "bound": "tensor", "achieved": bwd_tflops,
-                         "peak": pk["tflops"], "unit": "TFLOP/s", "frac": bwd_tflops / pk["tflops"],
-                         "traffic": ncu_traffic("attn_bwd_kernel")},
-            "merge": merge,
-            "softmax_xent": xent,
-            "ring_steps_cfg3_4_5": ring,
             "full_configs": full,
+            "ring_steps_cfg3_4_5": ring,
             "hdp_naive_replay": hdp,
             "hdp_balance_replay": hdp_bal,
             "static_cp_baseline": static_cp,
             "offload_probe": offload,
+            "softmax_xent": xent,
+            "merge": merge,
+            "pct_of_bf16_peak": {"measured_burst": 100 * value / world / pk["tflops"],
+                                 "nominal_2250": 100 * value / world / 2250.0},
+            "roofline": {"kernel": "attn_bwd_kernel<128>", "bound": "tensor", "achieved": bwd_tflops,
+                         "peak": pk["tflops"], "unit": "TFLOP/s", "frac": bwd_tflops / pk["tflops"],
+                         "traffic": ncu_traffic("attn_bwd_kernel"),
+                         "kernels": {
+                             "bs_attn_fwd": {"ms": round(t_fwd, 4), "tflops": round(fwd_tflops, 1),
+                                             "frac": round(fwd_tflops / pk["tflops"], 4)},
+                             "bs_attn_bwd_prep": {"ms": round(t_prep, 4),
+                                                  "gbs": round(prep_bytes / t_prep / 1e6, 1)},
+                             "bs_attn_bwd": {"ms": round(t_bwd, 4), "tflops": round(bwd_tflops, 1),
+                                             "frac": round(bwd_tflops / pk["tflops"], 4)},
+                             "bs_attn_bwd_finish": {"ms": round(t_fin, 4),
+                                                    "gbs": round(fin_bytes / t_fin / 1e6, 1)}},
+                         "sustained": {"tflops": round(sus, 1), "seconds": round(ms_sus * 1e-3, 2),
+                                       "steps": n_sus,
+                                       "frac_of_sustained_peak": round(sus / world / pk["tflops_sustained"], 4)
+                                       if pk["tflops_sustained"] else None,
+                                       "frac_of_burst_peak": round(sus / world / pk["tflops"], 4),
+                                       "sm_mhz_median": sampler.median_between(t_sus0, t_sus1)},
+                         "merge_gbs": {k: v for k, v in merge["by_config"].items()}},
             "cpu_baseline": {"value": fl / dt / 1e12, "unit": "TFLOP/s", "cores": thr, "kind": "oracle",
                              "sample": f"{CPU_BASELINE_HEADS} of {Hq} heads of {WORKLOAD}, all "
                                        f"{rows} tokens, fwd+bwd, fp64, {dt:.1f} s"},
@@ -339,28 +407,69 @@ def run_ours(args, rank, world, local_rank):
 
 
 def bench_merge(B, torch, pk):
-    """bs_lse_merge on the cfg3-shaped partials: n = 8, 32768 rows x 64 heads x 128 (4.6 GB)."""
-    n, rows, Hq, D = 8, 32768, 64, 128
-    Os = [torch.randn((rows, Hq, D), device="cuda").to(torch.bfloat16) for _ in range(n)]
-    Ls = [torch.randn((Hq, rows), device="cuda") for _ in range(n)]
-    O, L = torch.empty_like(Os[0]), torch.empty_like(Ls[0])
-    sh = B.make_shape(Hq, 8, D, rows, rows)
-    for _ in range(3):
-        B.lse_merge(Os, Ls, sh, (0, rows), O, L)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    it = 10
-    e0.record()
-    for _ in range(it):
-        B.lse_merge(Os, Ls, sh, (0, rows), O, L)
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / it
-    nbytes = (n + 1) * rows * Hq * (2 * D + 4)
-    gbs = nbytes / (ms * 1e-3) / 1e9
-    return {"workload": "cfg3 partials: n=8, 32768 rows, 64 heads, D=128", "ms": ms, "bytes": nbytes,
-            "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm"], "unit": "GB/s",
-                         "frac": gbs / pk["hbm"], "frac_of_nominal_8000": gbs / 8000.0,
+    """bs_lse_merge on the partials of configs 3, 4, 5 (n = 8 / 4 / 64 parts; rows x heads 32768 x 64,
+    65536 x 32, 32768 x 48; D = 128), each next to two plain streaming probes with the same byte
+    counts and the merge's own load instruction (bs_hbm_probe): n input streams read
+    and one written (n : 1), and n + 1 streams only read.  The probes say what a read-dominated
+    kernel can reach on this part; the merge is reported against them and against the measured
+    copy bandwidth."""
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+
+    def timed(fn, it=10):
+        for _ in range(3):
+            fn()
+        a, b = ev(), ev()
+        a.record()
+        for _ in range(it):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / it
+
+    out, D = {}, 128
+    sink = torch.zeros(4, dtype=torch.uint8, device="cuda")
+    for cfg, n, rows, Hq in ((3, 8, 32768, 64), (4, 4, 65536, 32), (5, 64, 32768, 48)):
+        Os = [torch.randn((rows, Hq, D), device="cuda").to(torch.bfloat16) for _ in range(n)]
+        Ls = [torch.randn((Hq, rows), device="cuda") for _ in range(n)]
+        O, L = torch.empty_like(Os[0]), torch.empty_like(Ls[0])
+        sh = B.make_shape(Hq, 8, D, rows, rows)
+        ms = timed(lambda: B.lse_merge(Os, Ls, sh, (0, rows), O, L), 10 if n < 64 else 4)
+        ms_alias = timed(lambda: B.lse_merge(Os, Ls, sh, (0, rows), Os[0], Ls[0]), 10 if n < 64 else 4)
+        nbytes = (n + 1) * rows * Hq * (2 * D + 4)
+        ms_n1 = timed(lambda: B.hbm_probe(Os, O, sink), 10 if n < 64 else 4)
+        ms_rd = timed(lambda: B.hbm_probe(Os + [O], None, sink), 10 if n < 64 else 4)
+        pbytes = (n + 1) * rows * Hq * 2 * D
+        gbs = nbytes / ms / 1e6
+        out[f"cfg{cfg}"] = {"n_parts": n, "rows": rows, "heads": Hq, "ms": round(ms, 4), "bytes": nbytes,
+                            "gbs": round(gbs, 1), "gbs_output_aliases_part0": round(nbytes / ms_alias / 1e6, 1),
+                            "probe_n_to_1_gbs": round(pbytes / ms_n1 / 1e6, 1),
+                            "probe_pure_read_gbs": round(pbytes / ms_rd / 1e6, 1),
+                            "frac_of_n_to_1_probe": round(gbs / (pbytes / ms_n1 / 1e6), 4),
+                            "frac_of_measured_copy": round(gbs / pk["hbm"], 4),
+                            "frac_of_nominal_8000": round(gbs / 8000.0, 4)}
+        del Os, Ls, O, L
+        torch.cuda.empty_cache()
+    c3 = out["cfg3"]
+    return {"workload": "partials of cfg3 / cfg4 / cfg5, D = 128; probes = bs_hbm_probe, same bytes",
+            "by_config": out,
+            "roofline": {"bound": "hbm", "achieved": c3["gbs"], "peak": pk["hbm"], "unit": "GB/s",
+                         "frac": c3["gbs"] / pk["hbm"], "frac_of_nominal_8000": c3["gbs"] / 8000.0,
                          "traffic": ncu_traffic("lse_merge_kernel")}}
+
+
+def tile_area_ratio(w):
+    """Pairs the attention kernels COMPUTE on this workload / pairs that are visible (and counted):
+    masked halves of diagonal tiles and ragged document tails earn nothing ("FLOPs
+    proportional to the areas of attention mask").  Both kernels visit every (128-row query tile,
+    128-key block) pair of a document with at least one visible element, whole.  Whole documents
+    (cp = 1) only."""
+    computed = vis = 0
+    for L, cp, _ in w.seqs:
+        assert cp == 1
+        n = -(-L // 128)
+        vis += L * (L + 1) // 2
+        computed += 128 * 128 * (n * (n + 1) // 2)
+    return round(computed / vis, 4)
 
 
 def bench_softmax_xent(B, torch, pk):
@@ -523,18 +632,78 @@ def bench_ring_steps(B, torch, workloads, pk):
     return out
 
 
+def run_plumbing(args, rank, world):
+    """The multi-rank launch path alone, on CPU (gloo): what --gpus N does around the timed region
+    - rendezvous, barrier, max over ranks, one line from rank 0 - with a host-only step (bs_plan
+    of cfg2) in place of the device work.  tests/test_dist_gloo.py drives it with 2 ranks."""
+    import torch.distributed as dist
+    from paper_2502_21231_b200 import binding as B
+    from paper_2502_21231_b200 import dist_util as DU
+    if world > 1:
+        dist.init_process_group("gloo")
+    else:
+        dist = None
+    w = cfg2()
+    for _ in range(max(args.warmup, 1)):
+        B.plan(w.seqs)
+    if dist:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        pl = B.plan(w.seqs)
+    ms = (time.perf_counter() - t0) * 1e3
+    (ms_max,) = DU.max_over_ranks(dist, [ms], "cpu")
+    if dist:
+        dist.barrier()
+    if rank == 0:
+        print(json.dumps({"impl": "plumbing", "metric": "bs_plan calls/s (host only)",
+                          "value": DU.whole_job_rate(args.steps, world, ms_max), "unit": "calls/s",
+                          "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 1),
+                          "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+                          "scaling": "weak", "q_rows": pl["q_rows"], "gpu_launches": 0}))
+    if dist:
+        dist.destroy_process_group()
+
+
+def launch_ranks(args):
+    """--gpus N > 1 without a launcher: start N ranks of this script under torch.distributed.run
+    (one process per GPU, rendezvous on 127.0.0.1) and pass their output through."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+           f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1", "--master-port", str(port),
+           os.path.abspath(__file__), "--gpus", str(args.gpus), "--steps", str(args.steps),
+           "--warmup", str(args.warmup), "--impl", args.impl] + (["--only-step"] if args.only_step else [])
+    return subprocess.call(cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "plumbing"])
+    ap.add_argument("--only-step", action="store_true",
+                    help="time the cfg2 step only (no sustained / e2e / merge / replay / oracle legs): "
+                         "the short command the ncu captures under profiles/ are taken with")
     args = ap.parse_args()
+    if args.impl != "reference" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(launch_ranks(args))
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     local_rank = int(os.environ.get("LOCAL_RANK", 0))
     if args.impl == "reference":
         run_reference(args, rank)
+    elif args.impl == "plumbing":
+        run_plumbing(args, rank, world)
     else:
+        if world > 1:
+            # NCCL only carries the barrier and the max over ranks; its communicator log stays on
+            # so that the number of ranks that really joined can be read from the run's output
+            os.environ.setdefault("NCCL_DEBUG", "INFO")
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         run_ours(args, rank, world, local_rank)
 
 

@@ -18,6 +18,15 @@
  *     host memory.  The library never allocates or frees device memory, and never synchronises
  *     the device: all device work is enqueued on `stream` (a cudaStream_t passed as void*; NULL =
  *     the legacy default stream).  Host arrays may be freed as soon as the call returns.
+ *     bs_attn_fwd / bs_attn_bwd stage their work-item tables in pinned host memory owned by the
+ *     library (a ring of 64 slots, allocated on first use, never freed) and copy them with one
+ *     DMA on `stream`; the host waits only when 64 such copies are still in flight.  Because the
+ *     slots are reused, these two calls must not be captured into a CUDA graph.
+ *   - Every argument check (shapes, ranges, segment consistency, workspace, alignment of every
+ *     pointer and stride, the device) is made before anything is enqueued: a call that returns
+ *     an error has written nothing.
+ *   - Rows of the buffers that no segment of a call references may hold anything, NaN and Inf
+ *     included (fixed-capacity or uninitialised padding): they never reach a result.
  *   - Tensors: Q, O, dO, dQ are [q_rows][n_q_heads][head_dim] bf16 with dim stride 1, head stride
  *     head_dim and row stride q_row_stride elements.  K, V, dK, dV are
  *     [kv_rows][n_kv_heads][head_dim] bf16 with row stride kv_row_stride.  LSE and delta are fp32,
@@ -40,7 +49,9 @@ extern "C" {
 typedef enum {
   BS_OK = 0,
   BS_ERR_INVALID_ARG = -1, /* null pointer, bad range, bad stride, inconsistent segments */
-  BS_ERR_UNSUPPORTED = -2, /* head_dim not in {64,128}, device is not sm_100 */
+  BS_ERR_UNSUPPORTED = -2, /* head_dim not in {64,128}; more than 2^30 - 1024 rows in a buffer; the
+                              current device is not compute capability 10.0 (checked by every
+                              device call before anything is enqueued) */
   BS_ERR_WORKSPACE = -3,   /* workspace null / too small / misaligned */
   BS_ERR_CUDA = -4,        /* a CUDA runtime/driver call failed; text from cudaGetErrorString */
   BS_ERR_HOST_OOM = -5
@@ -76,7 +87,11 @@ typedef struct {
  * keys = rows [k_begin,k_end) of THIS call's K/V buffers.  With a, b the 0-based indices inside
  * the two ranges, key b is visible to query a iff  b <= a + causal_offset.
  * Two segments of one call have identical or disjoint q ranges; a row's softmax runs over the
- * union of the visible keys of every segment that contains the row. */
+ * union of the visible keys of every segment that contains the row.  bs_attn_bwd additionally
+ * needs the k ranges of two segments to be identical or disjoint (it owns dK / dV per key range;
+ * bs_plan's segments satisfy both rules).  causal_offset may be any int32: offsets >= k_len - 1
+ * mean "every key", offsets <= -q_len "no key" (INT32_MAX / INT32_MIN are fine); the library
+ * clamps it to [-q_len, k_len], which leaves the mask unchanged. */
 typedef struct {
   int32_t q_begin, q_end;
   int32_t k_begin, k_end;
@@ -296,6 +311,16 @@ bs_status_t bs_lse_merge(int32_t n_parts, const void* const* O_parts,
 bs_status_t bs_softmax_xent(const void* logits, const int32_t* labels, int32_t n_tokens,
                             int32_t vocab, int64_t row_stride, float grad_scale, float* loss,
                             void* dlogits, void* stream);
+
+/* Measurement aid: the HBM rate a read-dominated streaming kernel can reach on
+ * this device, with the merge's own access pattern - n_in input streams of bytes_per_stream bytes
+ * each, read with 16-byte loads and combined word by word (XOR), then written to `out` (n : 1,
+ * the merge's shape) or, with out == NULL, only read (pure-read ceiling).  in: HOST array of n_in
+ * DEVICE pointers; out: device or NULL; sink: device, 4 bytes, never written in practice (it keeps
+ * the pure-read loads alive).  1 <= n_in <= BS_MAX_MERGE_PARTS; sizes and pointers 16-byte
+ * aligned.  bench.py reports bs_lse_merge against it. */
+bs_status_t bs_hbm_probe(int32_t n_in, const void* const* in, void* out, void* sink,
+                         size_t bytes_per_stream, void* stream);
 
 /* Number of kernels this library has launched on the calling thread since the last reset
  * (bench.py's "gpu_launches"). */

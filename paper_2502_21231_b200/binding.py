@@ -118,6 +118,7 @@ lib.bs_attn_bwd.argtypes = [_P(Shape), _vp, _vp, _vp, _vp, _vp, _vp, _P(Seg), _i
 lib.bs_attn_bwd_finish.argtypes = [_P(Shape), _vp, _vp, _vp]
 lib.bs_lse_merge.argtypes = [_i32, _P(_vp), _P(_vp), _P(Shape), _i32, _i32, _vp, _vp, _vp]
 lib.bs_softmax_xent.argtypes = [_vp, _vp, _i32, _i32, _i64, ctypes.c_float, _vp, _vp, _vp]
+lib.bs_hbm_probe.argtypes = [_i32, _P(_vp), _vp, _vp, _sz, _vp]
 lib.bs_launch_count.restype = _i64
 lib.bs_launch_count_reset.restype = None
 
@@ -130,6 +131,7 @@ EXPORTS = ["bs_status_string", "bs_last_error", "bs_version", "bs_plan", "bs_pla
            "bs_balance_exec_times", "bs_balance_makespan", "bs_balance_n_microbatches",
            "bs_balance_microbatch", "bs_balance_destroy", "bs_attn_workspace_bytes", "bs_attn_fwd",
            "bs_attn_bwd_prep", "bs_attn_bwd", "bs_attn_bwd_finish", "bs_lse_merge", "bs_softmax_xent",
+           "bs_hbm_probe",
            "bs_launch_count", "bs_launch_count_reset"]
 
 
@@ -297,6 +299,15 @@ def softmax_xent(logits, labels, grad_scale, loss, dlogits, vocab=None):
     _check(lib.bs_softmax_xent(_ptr(logits), _ptr(labels), T, stride if vocab is None else vocab,
                                stride, float(grad_scale), _ptr(loss), _ptr(dlogits), _stream()),
            "bs_softmax_xent")
+
+
+def hbm_probe(ins, out, sink):
+    """bs_hbm_probe on torch device tensors: ins = list of equally sized tensors, out = tensor of
+    that size or None (pure read), sink = a 4-byte device tensor."""
+    n = len(ins)
+    arr = (_vp * n)(*[t.data_ptr() for t in ins])
+    _check(lib.bs_hbm_probe(n, arr, _ptr(out), _ptr(sink), ins[0].numel() * ins[0].element_size(),
+                            _stream()), "bs_hbm_probe")
 
 
 def launch_count():

@@ -37,6 +37,9 @@
 #include "sched.cuh"
 #include "worklist.h"
 
+#define BS_TRACE_KERNEL_BWD
+#include "trace.cuh"
+
 namespace {
 
 using namespace bs;
@@ -52,23 +55,19 @@ using UnitConsumer = UnitConsumerT<kBwdSchedSlots>;
 constexpr int kSchedRingBytes = SchedRing::kBytes;
 
 constexpr int kBwdThreads = 512;   // 2 compute WGs, auxiliary WG (MMA, TMA, scheduler), dQ drain WG
-constexpr int kRegsCompute = 144, kRegsAux = 64, kRegsDrain = 160;  // 2*144 + 64 + 160 = 4*128
+#ifndef BS_BWD_REGS_C
+#define BS_BWD_REGS_C 144
+#define BS_BWD_REGS_A 64
+#define BS_BWD_REGS_D 160
+#endif
+// setmaxnreg split: compute, auxiliary, drain warpgroups: 2 c + a + d = 4 * 128
+constexpr int kRegsCompute = BS_BWD_REGS_C, kRegsAux = BS_BWD_REGS_A, kRegsDrain = BS_BWD_REGS_D;
+static_assert(2 * kRegsCompute + kRegsAux + kRegsDrain == 512, "register split");
 constexpr int kComputeThreads = 256;
 #ifndef BS_BWD_EMU
 #define BS_BWD_EMU 0  // (1 of 4 was worth ~1 % before the dQ boxes became whole lines; now 0 is 2 % faster on cfg2)
 #endif
 constexpr int kBwdEmuOf4 = BS_BWD_EMU;  // of every 4 column pairs, this many take the FMA-pipe exp2
-
-#ifdef BS_BWD_TRACE
-// debug build only: clock64() stamps of CTA 0: [role][event][iteration]
-__device__ long long g_bwd_trace[3][10][512];
-#define TRACE(role, ev, it)                                                    \
-  do {                                                                         \
-    if (blockIdx.x == 0 && (it) < 512) g_bwd_trace[role][ev][it] = clock64();  \
-  } while (0)
-#else
-#define TRACE(role, ev, it) do {} while (0)
-#endif
 
 struct BwdParams {
   SchedView sv;     // units = key-tile items x n_kv_heads
@@ -202,24 +201,6 @@ __device__ __forceinline__ void warp_arrive(uint64_t* bar) {
   if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
 }
 
-// Rows [v, 128) of a 128-row tile (TMA layout: one 16 KB box of 128-byte rows per 64 columns) are
-// set to zero by the 256 compute threads.  TMA loads whole boxes, so behind a ragged range end the
-// tile holds whatever follows in the caller's buffer - another document, or uninitialised rows
-// with NaN / Inf.  Masked P and dS are exactly 0, but 0 x NaN inside an MMA's contraction would
-// still poison every output row of the tile; the rows a contraction runs over must be finite.
-// (The 128-byte swizzle permutes 16-byte chunks inside a row: zeroing whole rows needs no index
-// arithmetic.)
-template <int D>
-__device__ __forceinline__ void zero_tile_rows(uint8_t* tile, int v, int tid256) {
-  constexpr int kChunksPerRow = D / 8;  // 16-byte chunks of one row over all column boxes
-  const int total = (kTile - v) * kChunksPerRow;
-  for (int i = tid256; i < total; i += kComputeThreads) {
-    const int row = v + i / kChunksPerRow, cc = i % kChunksPerRow;
-    *reinterpret_cast<uint4*>(tile + (cc / 8) * (kTile * 128) + row * 128 + (cc % 8) * 16) =
-        make_uint4(0, 0, 0, 0);
-  }
-}
-
 template <int D>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
@@ -296,7 +277,26 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
   if (warp >= 8 && warp < 12) setmaxnreg_dec<kRegsAux>();
   if (warp == 9) {
     // ============================ TMA producer + LSE/delta staging ============================
+    // Ragged tiles - the last key tile of a key range, the last query tile of a query range -
+    // are loaded through tensor maps whose row extent ends at the range end (host-built, in the
+    // workspace): TMA zero-fills the rows past it.  A whole 128-row box through the buffer-wide
+    // map would bring in whatever follows in the caller's buffer - another document, or
+    // uninitialised rows with NaN / Inf - and 0 (masked P, dS) x NaN inside an MMA's contraction
+    // would poison every output row of the tile.
+    // A tensor map in global memory must be fenced by the thread that uses it (the workspace
+    // address held other maps in earlier launches).  A fence costs ~360 cycles and the loads of
+    // ragged tiles sit on the iteration's critical path (single-buffered dO), so every clipped
+    // map is OWNED by one lane of this warp - lane 1 + index % 31 - which fences it once, up
+    // front, and issues every load that goes through it; lane 0 issues all other loads.
     uint32_t item_n = 0, it_n = 0;  // items / iterations issued so far (ring phases)
+    const CUtensorMap* clips_q = p.sv.tmaps;                           // [2 i] Q, [2 i + 1] dO
+    const CUtensorMap* clips_k = p.sv.tmaps + 2 * p.sv.n_span_clips;   // [2 j] K, [2 j + 1] V
+    if (lane > 0) {
+      for (int c = lane - 1; c < p.sv.n_span_clips + p.sv.n_item_clips; c += 31) {
+        tensormap_acquire(clips_q + 2 * c);
+        tensormap_acquire(clips_q + 2 * c + 1);
+      }
+    }
     UnitConsumer cons{sched};  // lane 0 consumes; the other lanes read the slot after it
     while (true) {
       Unit u;
@@ -316,26 +316,34 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       // buffers free up well before the previous unit ends, whereas V is only released at that
       // unit's last dP^T MMA and K at its last dQ MMA.  K/V then stream in under the previous
       // unit's tail (dS, dK/dQ, the dQ drain and the dK/dV epilogue).
+      const int kclip = it.tile_blocks[0];  // bwd: clipped K / V maps of this key tile, or -1
+      const CUtensorMap* mK = kclip >= 0 ? clips_k + 2 * kclip : &tmK;
+      const CUtensorMap* mV = kclip >= 0 ? mK + 1 : &tmV;
+      const int own_k = kclip >= 0 ? 1 + (p.sv.n_span_clips + kclip) % 31 : 0;
       auto load_kv = [&]() {
         TRACE(2, 8, it_n);  // the producer is ready to load this unit's K / V
         mbar_wait(v_empty, (item_n & 1) ^ 1);
         mbar_arrive_expect_tx(v_full, L::kTileBytes);
         for (int half = 0; half < D / 64; ++half)
-          tma_load_3d(smem + L::kVOff + half * (kTile * 128), &tmV, v_full, half * 64, g, it.row0);
+          tma_load_3d(smem + L::kVOff + half * (kTile * 128), mV, v_full, half * 64, g, it.row0);
         mbar_wait(k_empty, (item_n & 1) ^ 1);
         TRACE(2, 9, it_n);  // K requested
         mbar_arrive_expect_tx(k_full, L::kTileBytes);
         for (int half = 0; half < D / 64; ++half)
-          tma_load_3d(smem + L::kKOff + half * (kTile * 128), &tmK, k_full, half * 64, g, it.row0);
+          tma_load_3d(smem + L::kKOff + half * (kTile * 128), mK, k_full, half * 64, g, it.row0);
       };
       bool kv_pending = true;
       for (; !wk.done(); wk.next(), ++it_n) {
         const int st = it_n & 1, h = g * p.group + wk.hi, qrow = wk.q_row();
+        const bool qclip = wk.sp.clip >= 0 && wk.sp.len - wk.qi * kTile < kTile;
+        const CUtensorMap* mQ = qclip ? clips_q + 2 * wk.sp.clip : &tmQ;
+        const CUtensorMap* mDO = qclip ? mQ + 1 : &tmDO;
+        const int own_q = qclip ? 1 + wk.sp.clip % 31 : 0;
         mbar_wait(&q_empty[st], ((it_n >> 1) & 1) ^ 1);
-        if (lane == 0) {
+        if (lane == own_q) {
           mbar_arrive_expect_tx(&q_full[st], L::kTileBytes);
           for (int half = 0; half < D / 64; ++half)
-            tma_load_3d(smem + L::kQOff + st * L::kTileBytes + half * (kTile * 128), &tmQ,
+            tma_load_3d(smem + L::kQOff + st * L::kTileBytes + half * (kTile * 128), mQ,
                         &q_full[st], half * 64, h, qrow);
         }
         // -lse*log2e (-inf for rows outside the query range) and -delta*scale
@@ -348,12 +356,15 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           delta_s[st * kTile + c] = ok ? -p.delta[idx] * p.scale : 0.f;
         }
         mbar_arrive(&q_full[st]);
-        if (lane == 0) {
+        if (lane == own_q) {
           mbar_wait(do_empty, (it_n & 1) ^ 1);
           mbar_arrive_expect_tx(do_full, L::kTileBytes);
           for (int half = 0; half < D / 64; ++half)
-            tma_load_3d(smem + L::kDOOff + half * (kTile * 128), &tmDO, do_full, half * 64, h, qrow);
-          if (kv_pending) load_kv();
+            tma_load_3d(smem + L::kDOOff + half * (kTile * 128), mDO, do_full, half * 64, h, qrow);
+        }
+        if (kv_pending) {
+          __syncwarp();  // K / V go out behind the first dO, whichever lanes issue them
+          if (lane == own_k) load_kv();
         }
         kv_pending = false;
         __syncwarp();
@@ -526,10 +537,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
       }
       uint32_t pk[32];  // P^T of this thread as the tensor core sees it (bf16 pairs), kept for dS
       bool first = true;
-      bool full_it = false;      // mask of the current iteration, kept for the dS step
-      int c_min_it = 0, c_max_it = 0;
-      const int tid256 = threadIdx.x & 255;
-      const int vk = it.range_len - it.local0;  // valid keys of the tile (>= 128: all)
 
       auto compute_p = [&](const BwdWalker& k, uint32_t n) {
         mbar_wait(s_full, n & 1);
@@ -547,28 +554,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                           a0 + 64 <= k.sp.len;
         const int c_min = key_ok ? b - k.sp.off - a0 : (1 << 30);
         const int c_max = k.sp.len - a0;
-        full_it = full;
-        c_min_it = c_min;
-        c_max_it = c_max;
-        // Ragged tiles: rows past the range end must not carry NaN / Inf into a contraction.
-        // K rows past the key range (the dQ MMA sums over keys): once per unit, K has landed
-        // (S^T of this iteration is complete).  Q and dO rows past the query range (the dK and dV
-        // MMAs sum over queries): Q has landed with S^T; dO's own barrier is awaited here, the dV
-        // MMA waits for this warp's p_full arrival below.  S^T / dP^T themselves are elementwise
-        // in those rows and masked by select.
-        bool zeroed = false;
-        if (first && vk < kTile) {
-          zero_tile_rows<D>(smem + L::kKOff, vk, tid256);
-          zeroed = true;
-        }
-        const int vq = k.sp.len - k.qi * kTile;  // valid queries of the tile (>= 128: all)
-        if (vq < kTile) {
-          mbar_wait(do_full, n & 1);
-          zero_tile_rows<D>(smem + L::kQOff + (n & 1) * L::kTileBytes, vq, tid256);
-          zero_tile_rows<D>(smem + L::kDOOff, vq, tid256);
-          zeroed = true;
-        }
-        if (zeroed) fence_proxy_async_smem();
         const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
         // two copies of the loop: unmasked pieces (nearly all of them) run branch- and
         // predicate-free straight-line code
@@ -616,30 +601,23 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           }
           const float2* nd2 = reinterpret_cast<const float2*>(delta_s + (it_n & 1) * kTile + wg * 64);
           const float2 s2 = make_float2(p.scale, p.scale);
-          // two copies, as for P: masked pieces build dS by select (P = 0 times a dP from rows
-          // past a range end - possibly NaN - must give 0), unmasked ones stay straight-line code
-          auto ds_all = [&](auto masked) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {  // 8 queries = one 16-byte chunk of the dS^T row
-              uint32_t w4[4];
+          for (int j = 0; j < 8; ++j) {  // 8 queries = one 16-byte chunk of the dS^T row
+            uint32_t w4[4];
 #pragma unroll
-              for (int e = 0; e < 4; ++e) {
-                const int i = 4 * j + e;
-                const float2 t = fma2(make_float2(__uint_as_float(dp[2 * i]), __uint_as_float(dp[2 * i + 1])),
-                                      s2, nd2[i]);
-                // P widened exactly from the bf16 pair the dV MMA used
-                float2 d = mul2(make_float2(__uint_as_float(pk[i] << 16),
-                                            __uint_as_float(pk[i] & 0xffff0000u)), t);
-                if (decltype(masked)::value) {
-                  if (2 * i < c_min_it || 2 * i >= c_max_it) d.x = 0.f;
-                  if (2 * i + 1 < c_min_it || 2 * i + 1 >= c_max_it) d.y = 0.f;
-                }
-                w4[e] = pack_bf16(d.x, d.y);
-              }
-              *reinterpret_cast<uint4*>(ds_row + ((j ^ (r & 7)) * 16)) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+            for (int e = 0; e < 4; ++e) {
+              const int i = 4 * j + e;
+              const float2 t = fma2(make_float2(__uint_as_float(dp[2 * i]), __uint_as_float(dp[2 * i + 1])),
+                                    s2, nd2[i]);
+              // P widened exactly from the bf16 pair the dV MMA used.  Masked P is exactly 0 and
+              // t is finite everywhere (rows past a range end are zero-filled by TMA, see the
+              // producer), so masked dS is exactly 0 without a select.
+              const float2 d = mul2(make_float2(__uint_as_float(pk[i] << 16),
+                                                __uint_as_float(pk[i] & 0xffff0000u)), t);
+              w4[e] = pack_bf16(d.x, d.y);
             }
-          };
-          if (full_it) ds_all(std::false_type{}); else ds_all(std::true_type{});
+            *reinterpret_cast<uint4*>(ds_row + ((j ^ (r & 7)) * 16)) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
+          }
         }
         if (r == 0) TRACE(wg, 9, it_n);
         fence_proxy_async_smem();
@@ -728,12 +706,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
 }  // namespace
 
-#ifdef BS_BWD_TRACE
-extern "C" int bs_debug_bwd_trace(long long* host_out) {
-  return (int)cudaMemcpyFromSymbol(host_out, g_bwd_trace, sizeof(g_bwd_trace));
-}
-#endif
-
 extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, const void* K,
                                    const void* V, const void* dO, const float* LSE_final,
                                    const float* delta, const bs_seg_t* segs, int32_t n_segs,
@@ -754,11 +726,24 @@ extern "C" bs_status_t bs_attn_bwd(const bs_attn_shape_t* shape, const void* Q, 
   rc = bs::build_bwd_tables(segs, n_segs, shape->q_rows, shape->kv_rows, shape->n_kv_heads, &tb);
   if (rc != BS_OK) return rc;
   bs::WsLayout L;
-  rc = bs::check_workspace(tb, ws, ws_bytes, &L);
+  const size_t n_qc = tb.clip_span_rows.size(), n_kc = tb.clip_item_rows.size();
+  rc = bs::check_workspace(tb, 2 * (n_qc + n_kc) * bs::kTensorMapBytes, ws, ws_bytes, &L);
   if (rc != BS_OK) return rc;
   rc = bs::check_device();
   if (rc != BS_OK) return rc;
   const int D = shape->head_dim;
+  // Q / dO maps cut at every query range end and K / V maps cut at every key range end that is
+  // not tile-aligned (TMA zero-fills past the end): [2 i] Q, [2 i + 1] dO, then [2 j] K, [2 j + 1] V
+  rc = bs::append_clipped_maps(&tb, 0, 2, tb.clip_span_rows, Q, D, shape->n_q_heads, shape->q_row_stride);
+  if (rc == BS_OK)
+    rc = bs::append_clipped_maps(&tb, 1, 2, tb.clip_span_rows, dO, D, shape->n_q_heads, shape->q_row_stride);
+  if (rc == BS_OK)
+    rc = bs::append_clipped_maps(&tb, 2 * n_qc, 2, tb.clip_item_rows, K, D, shape->n_kv_heads,
+                                 shape->kv_row_stride);
+  if (rc == BS_OK)
+    rc = bs::append_clipped_maps(&tb, 2 * n_qc + 1, 2, tb.clip_item_rows, V, D, shape->n_kv_heads,
+                                 shape->kv_row_stride);
+  if (rc != BS_OK) return rc;
   CUtensorMap tmQ, tmK, tmV, tmDO, tmDQ, tmDK, tmDV;
   rc = bs::make_tensor_map_3d(&tmQ, Q, 2, D, shape->n_q_heads, shape->q_rows, shape->q_row_stride,
                               64, bs::kTile, 128);

@@ -1,18 +1,24 @@
 // attn_fwd.cu — bs_attn_fwd: one Q-chunk x KV-chunk step of packed varlen / zigzag-CP causal
 // attention on sm_100a (SURVEY.md 8(a) a2+a3; flash attention = exact attention).
 //
-// Kernel shape (one persistent CTA per SM, 384 threads, registers re-split by setmaxnreg):
-//   warps 0-3  softmax warpgroup of Q tile 0   (thread r <-> row r of the 128-row tile)
-//   warps 4-7  softmax warpgroup of Q tile 1
-//   warps 8,10 MMA issuers of Q tile 0 / 1 (one lane each): tcgen05.mma, accumulators in TMEM
-//   warp  9    TMA producer + scheduler: Q per unit and tile, K/V blocks through a 4-stage ring
+// Kernel shape: one persistent CTA per SM, 640 threads at 96 registers, 1 CTA / SM:
+//   warps 0-15  softmax: warpgroup g = warp / 4 works on Q tile t = g / 2, key columns
+//               [64 hf, 64 hf + 64) of every block with hf = g % 2 - two threads share a row (row r
+//               of the tile <-> threads r and 128 + r of the tile's 256), the row maximum and the
+//               row sum are exchanged through shared memory
+//   warp  16/18 MMA issuers of Q tile 0 / 1 (one elected lane each): tcgen05.mma, accumulators in
+//               TMEM; a turn lock keeps the two tiles' batches half a period apart
+//   warp  17    lane 0: TMA producer (Q per unit and tile, K/V blocks through a 4-stage ring, the
+//               accumulator-clearing stores)
+//   warp  19    scheduler (sched.cuh): pulls units from the global cursor into a shared-memory ring
 // A work item is (up to 256 query rows = two 128-row tiles of one query range, one query head).
 // TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,256+D) O1 [384,384+D); P (bf16) of 16 keys
-// overwrites the first 8 of the 16 S columns of those keys.  Per tile the chain is S(b) -> softmax -> P(b) -> PV(b), S(b+1);
-// the two tiles run this chain independently, so the softmax of one overlaps the MMAs of the
-// other, and P is handed over in two halves so that PV starts under the second half's exponentials.  Softmax is fp32 with exp2,
-// a lazily updated running max (rescale of O only when the max grew by more than 2^8) and the
-// row sum kept in fp32; O is normalised and written as bf16 with LSE = m ln2 + ln l at the end.
+// overwrites the first 8 of the 16 S columns of those keys.  Per tile the chain is S(b) -> softmax
+// -> P(b) -> PV(b), S(b+1); the two tiles run it independently, so the softmax of one overlaps
+// the MMAs of the other, and P is handed over in four 16-column chunks (order 3, 2, 0, 1) so that
+// PV starts under the remaining exponentials.  Softmax is fp32 with exp2, a lazily updated
+// running max (O is rescaled only when the max grew by more than 2^8) and the row sum kept in
+// fp32; O is normalised and written as bf16 with LSE = m ln2 + ln l at the end.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -24,6 +30,9 @@
 #include "ptx.cuh"
 #include "sched.cuh"
 #include "worklist.h"
+
+#define BS_TRACE_KERNEL_FWD
+#include "trace.cuh"
 
 namespace {
 
@@ -48,19 +57,8 @@ constexpr float kRescaleThreshold = 8.f;  // log2 units
 #define BS_FWD_EMU 1
 #endif
 constexpr int kEmuOf4 = BS_FWD_EMU;  // of every 4 column pairs, this many take the FMA-pipe exp2
-
-#ifdef BS_FWD_TRACE
-// debug build only: per-event clock64() stamps of CTA 0 (role, event) x iteration
-__device__ long long g_fwd_trace[4][8][256];
-__device__ long long g_fwd_utrace[5][8][64];  // per unit: softmax thread 0 of tile t
-#define UTRACE(t, ev, n) do { if (blockIdx.x == 0 && (n) < 64) g_fwd_utrace[t][ev][n] = clock64(); } while (0)
-#define TRACE(role, ev, it)                                                    \
-  do {                                                                         \
-    if (blockIdx.x == 0 && (it) < 256) g_fwd_trace[role][ev][it] = clock64();  \
-  } while (0)
-#else
-#define TRACE(role, ev, it) do {} while (0)
-#define UTRACE(t, ev, n) do {} while (0)
+#ifndef BS_FWD_LASTLOCK
+#define BS_FWD_LASTLOCK 1  // 0: a unit's last PV chunk (no S MMA behind it) is issued without the turn lock
 #endif
 
 struct FwdParams {
@@ -227,7 +225,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
   if (warp == kTmaWarp && lane == 0) {
     *reinterpret_cast<uint32_t*>(smem + L::kLockOff) = 0;
-    sched_ring_init(sched, 4 * kTile + 3);  // 512 softmax threads + 2 MMA lanes + the TMA lane  // consumers: 512 softmax threads + 2 MMA lanes
+    sched_ring_init(sched, 4 * kTile + 3);  // 512 softmax threads + 2 MMA lanes + the TMA lane
     for (int t = 0; t < 2; ++t) {
       mbar_init(&q_full[t], 1);
       mbar_init(&q_empty[t], 1);
@@ -260,6 +258,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (warp == kTmaWarp && lane == 0) {
       // ===================================== TMA producer =====================================
       uint32_t q_ph[2] = {0, 0};
+      uint64_t fenced = 0;  // clipped tensor maps (index < 64) this thread has fenced
       Ring ring;
       UnitConsumer cons{sched};
       Unit u;
@@ -283,17 +282,28 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // last S MMA of the previous unit), then V of the first block and the rest.  V stages are
         // only released at PV MMAs, i.e. late in the previous unit: nothing S(0) needs may queue
         // behind them.
-        auto load_kv = [&](int kv, int krow) {
+        // The V block that runs past the end of its key range is loaded through a tensor map whose
+        // row extent ends at the range end (host-built, in the workspace), so that TMA zero-fills
+        // the rows past it: a whole 128-row box through the buffer-wide map would bring in whatever
+        // follows in the caller's buffer (another document, or uninitialised rows with NaN / Inf),
+        // and P = 0 times NaN inside the PV contraction would poison every row of O.  A tensor map
+        // in global memory must be fenced by the thread that uses it (~360 cycles): once per map
+        // and CTA (bit mask; maps beyond the 64th are fenced at every use).
+        auto load_kv = [&](int krow, const CUtensorMap* m, int clip) {
+          if (clip >= 0 && (clip >= 64 || !((fenced >> clip) & 1))) {
+            tensormap_acquire(m);
+            if (clip < 64) fenced |= 1ull << clip;
+          }
           mbar_wait(&kv_empty[ring.stage], ring.phase ^ 1);
           mbar_arrive_expect_tx(&kv_full[ring.stage], L::kTileBytes);
           for (int half = 0; half < D / 64; ++half)
-            tma_load_3d(smem + L::kKVOff + ring.stage * L::kTileBytes + half * (kTile * 128),
-                        kv == 0 ? &tmK : &tmV, &kv_full[ring.stage], half * 64, g, krow);
+            tma_load_3d(smem + L::kKVOff + ring.stage * L::kTileBytes + half * (kTile * 128), m,
+                        &kv_full[ring.stage], half * 64, g, krow);
           ring.advance();
         };
         for (bool first = true; !wk.done(); wk.next(), first = false) {
           const int krow = wk.sp.begin + wk.j * kTile;
-          load_kv(0, krow);
+          load_kv(krow, &tmK, -1);
           if (first) {
             UTRACE(4, 1, un);
             for (int t = 0; t < 2; ++t) {
@@ -307,7 +317,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             &q_full[t], half * 64, h, it.row0 + wk.tile(t) * kTile);
             }
           }
-          load_kv(1, krow);
+          const int clip = (wk.sp.clip >= 0 && wk.sp.len - wk.j * kTile < kTile) ? wk.sp.clip : -1;
+          load_kv(krow, clip >= 0 ? p.sv.tmaps + clip : &tmV, clip);
           if (first) UTRACE(4, 4, un);
         }
         UTRACE(4, 5, un);
@@ -405,7 +416,9 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           // The batch [PV_t(b), S_t(b+1)] is issued under the turn lock: batches of the two tiles
           // enter the tensor pipe whole, one after the other, which keeps the tiles half a period
           // apart (softmax of one under the MMAs of the other) instead of drifting into phase.
-          while (atom_cas_shared(turn, 0u, 1u) != 0u) __nanosleep(20);
+          const bool locked = BS_FWD_LASTLOCK || has_next;  // (experiment switch)
+          if (locked)
+            while (atom_cas_shared(turn, 0u, 1u) != 0u) __nanosleep(20);
           if (lane == 0) TRACE(2 + t, 1, tr_it);
           if (cur.active(t)) {
             {
@@ -420,7 +433,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             release(k_stage);
           }
           if (lane == 0) TRACE(2 + t, 3, tr_it);
-          st_release_shared(turn, 0u);
+          if (locked) st_release_shared(turn, 0u);
           if (lane == 0) TRACE(2 + t, 4, tr_it);
           ++tr_it;
           if (!has_next) break;
@@ -445,7 +458,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
     uint32_t s_ph = 0, o_ph = 0;
     int tr_it = 0;
-    Ring ring;  // mirrors the producer's K/V ring: two stages (K, V) per visited block
     UnitConsumer cons{sched};
     Unit u;
     int un = -1;
@@ -466,19 +478,12 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           for (int c = 0; c < D / 16; ++c) reinterpret_cast<uint4*>(o_ptr)[c] = make_uint4(0, 0, 0, 0);
           if (hf == 0) p.LSE[(int64_t)h * p.lse_head_stride + grow] = -CUDART_INF_F;
         }
-        for (; !wk.done(); wk.next()) {  // the other tile's blocks still pass through the ring
-          ring.advance();
-          ring.advance();
-        }
         continue;
       }
       float m_used = -CUDART_INF_F;
       float2 l2 = make_float2(0.f, 0.f);
       int cnt = 0;
       for (; !wk.done(); wk.next()) {
-        ring.advance();  // K stage of this block
-        const uint32_t v_stage = ring.stage, v_phase = ring.phase;
-        ring.advance();
         if (!wk.active(t)) continue;
         mbar_wait(&s_full[t], s_ph);
         s_ph ^= 1;
@@ -537,24 +542,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         max16m(A, 32);
         max16m(B, 48);  // chunk 3 stays in B for pass 2
         if (r == 0) TRACE(t, 1, tr_it);
-        // Ragged key block: TMA loaded a whole 128-row V box, so the rows past the key range hold
-        // whatever follows in the caller's buffer (another document, or uninitialised rows with
-        // NaN / Inf).  P is exactly 0 there, but 0 x NaN inside the PV contraction would poison
-        // every row of O: the 256 softmax threads of this tile zero those V rows (both tiles do,
-        // with the same zeros) before the first chunk of P is handed over.
-        if (edge && b0 + kTile > wk.sp.len) {
-          const int vk = wk.sp.len - b0;
-          mbar_wait(&kv_full[v_stage], v_phase);
-          uint8_t* vt = smem + L::kKVOff + v_stage * L::kTileBytes;
-          constexpr int kChunksPerRow = D / 8;
-          const int total = (kTile - vk) * kChunksPerRow;
-          for (int i = (threadIdx.x & 255); i < total; i += 256) {
-            const int row = vk + i / kChunksPerRow, cc = i % kChunksPerRow;
-            *reinterpret_cast<uint4*>(vt + (cc / 8) * (kTile * 128) + row * 128 + (cc % 8) * 16) =
-                make_uint4(0, 0, 0, 0);
-          }
-          fence_proxy_async_smem();
-        }
         const float mx_half = fmaxf(mx0, mx1);
         // exchange the half-row maxima (slots alternate with the block parity; one barrier/block)
         xch_m[(cnt & 1) * 256 + hf * 128] = mx_half;
@@ -687,9 +674,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         p.LSE[(int64_t)h * p.lse_head_stride + grow] =
             l > 0.f ? m_used * 0.69314718055994531f + __logf(l) : -CUDART_INF_F;
       if (r == 0 && hf == 0) UTRACE(t, 4, un);
-#ifdef BS_FWD_TRACE
-      if (r == 0 && hf == 0 && blockIdx.x == 0 && un < 64) g_fwd_utrace[t][5][un] = tot;
-#endif
+      if (r == 0 && hf == 0) UTRACE_VALUE(t, 5, un, tot);
       tc_fence_before();
     }
   }
@@ -699,15 +684,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 }
 
 }  // namespace
-
-#ifdef BS_FWD_TRACE
-extern "C" int bs_debug_fwd_trace(long long* host_out) {
-  return (int)cudaMemcpyFromSymbol(host_out, g_fwd_trace, sizeof(g_fwd_trace));
-}
-extern "C" int bs_debug_fwd_utrace(long long* host_out) {
-  return (int)cudaMemcpyFromSymbol(host_out, g_fwd_utrace, sizeof(g_fwd_utrace));
-}
-#endif
 
 extern "C" {
 
@@ -744,11 +720,15 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
                             shape->n_q_heads, &tb);
   if (rc != BS_OK) return rc;
   bs::WsLayout L;
-  rc = bs::check_workspace(tb, ws, ws_bytes, &L);
+  rc = bs::check_workspace(tb, tb.clip_span_rows.size() * bs::kTensorMapBytes, ws, ws_bytes, &L);
   if (rc != BS_OK) return rc;
   rc = bs::check_device();
   if (rc != BS_OK) return rc;
   const int D = shape->head_dim;
+  // V maps cut at every key range end that is not tile-aligned (TMA zero-fills past the end)
+  rc = bs::append_clipped_maps(&tb, 0, 1, tb.clip_span_rows, V, D, shape->n_kv_heads,
+                               shape->kv_row_stride);
+  if (rc != BS_OK) return rc;
   CUtensorMap tmQ, tmK, tmV, tmZ;
   rc = bs::make_tensor_map_3d(&tmQ, Q, 2, D, shape->n_q_heads, shape->q_rows, shape->q_row_stride,
                               64, bs::kTile, 128);

@@ -14,6 +14,7 @@
 #include <cstring>
 #include <mutex>
 #include <new>
+#include <vector>
 
 #include "launch_utils.h"
 
@@ -79,9 +80,10 @@ bs_status_t set_max_smem_once(const void* func, int bytes, int kernel_slot) {
   return BS_OK;
 }
 
-bs_status_t check_workspace(const SchedTables& tb, const void* ws, size_t ws_bytes,
-                            WsLayout* layout) {
-  const WsLayout L = ws_layout(tb.items.size(), tb.spans.size(), tb.groups.size(), tb.fill.size());
+bs_status_t check_workspace(const SchedTables& tb, size_t tmap_bytes, const void* ws,
+                            size_t ws_bytes, WsLayout* layout) {
+  const WsLayout L = ws_layout(tb.items.size(), tb.spans.size(), tb.groups.size(), tb.fill.size(),
+                               tmap_bytes);
   BS_REQUIRE(ws != nullptr && ((uintptr_t)ws & 255) == 0, BS_ERR_WORKSPACE,
              "workspace is null or not 256-byte aligned");
   BS_REQUIRE(ws_bytes >= L.total, BS_ERR_WORKSPACE, "workspace too small: %zu < %zu bytes",
@@ -90,7 +92,28 @@ bs_status_t check_workspace(const SchedTables& tb, const void* ws, size_t ws_byt
   return BS_OK;
 }
 
-// [header | items | spans | groups | fill] -> workspace, one DMA from a pinned staging slot.
+bs_status_t append_clipped_maps(SchedTables* tb, size_t slot0, size_t slot_stride,
+                                const std::vector<int32_t>& end_rows, const void* base,
+                                int head_dim, int n_heads, int64_t row_stride_elems) {
+  static_assert(sizeof(CUtensorMap) == kTensorMapBytes, "CUtensorMap size");
+  try {
+    const size_t need = (slot0 + (end_rows.empty() ? 0 : (end_rows.size() - 1) * slot_stride + 1)) *
+                        kTensorMapBytes;
+    if (tb->tmaps.size() < need) tb->tmaps.resize(need);
+  } catch (const std::bad_alloc&) {
+    return fail(BS_ERR_HOST_OOM, "out of host memory building the clipped tensor maps");
+  }
+  for (size_t i = 0; i < end_rows.size(); ++i) {
+    CUtensorMap m;
+    bs_status_t rc = make_tensor_map_3d(&m, base, 2, head_dim, n_heads, end_rows[i],
+                                        row_stride_elems, 64, kTile, 128);
+    if (rc != BS_OK) return rc;
+    memcpy(tb->tmaps.data() + (slot0 + i * slot_stride) * kTensorMapBytes, &m, kTensorMapBytes);
+  }
+  return BS_OK;
+}
+
+// [header | items | spans | groups | fill | tensor maps] -> workspace, one DMA from a pinned slot.
 bs_status_t upload_tables(const SchedTables& tb, const WsLayout& L, void* ws, cudaStream_t st) {
   std::lock_guard<std::mutex> lock(g_mu);
   Slot& s = g_slots[g_next];
@@ -130,6 +153,7 @@ bs_status_t upload_tables(const SchedTables& tb, const WsLayout& L, void* ws, cu
     memcpy(s.host + L.spans_off, tb.spans.data(), tb.spans.size() * sizeof(Span));
   if (!tb.fill.empty())
     memcpy(s.host + L.fill_off, tb.fill.data(), tb.fill.size() * sizeof(RowRange));
+  if (!tb.tmaps.empty()) memcpy(s.host + L.tmaps_off, tb.tmaps.data(), tb.tmaps.size());
   BS_CUDA(cudaMemcpyAsync(ws, s.host, L.total, cudaMemcpyHostToDevice, st));
   BS_CUDA(cudaEventRecord(s.done, st));
   s.in_flight = true;

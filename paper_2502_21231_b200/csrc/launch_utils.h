@@ -34,8 +34,15 @@ bs_status_t check_device(int* device_out = nullptr);
 int sm_count();  // of the current device (after check_device)
 // cudaFuncAttributeMaxDynamicSharedMemorySize, set once per device and kernel (kernel_slot < 32)
 bs_status_t set_max_smem_once(const void* func, int bytes, int kernel_slot);
-// Workspace checks (null / alignment / size) and layout; enqueues nothing.
-bs_status_t check_workspace(const SchedTables& tb, const void* ws, size_t ws_bytes, WsLayout* layout);
+// Workspace checks (null / alignment / size) and layout; enqueues nothing.  tmap_bytes = size of
+// the clipped tensor maps the entry point is going to put into tb.tmaps.
+bs_status_t check_workspace(const SchedTables& tb, size_t tmap_bytes, const void* ws, size_t ws_bytes,
+                            WsLayout* layout);
+// Appends to tb->tmaps one tensor map per row in `end_rows`: the map of make_tensor_map_3d over
+// the same tensor with its row extent cut at that row (TMA zero-fills the rows past it).
+bs_status_t append_clipped_maps(SchedTables* tb, size_t slot0, size_t slot_stride,
+                                const std::vector<int32_t>& end_rows, const void* base,
+                                int head_dim, int n_heads, int64_t row_stride_elems);
 // Tables -> workspace on `st` from a pinned staging slot (no stream synchronisation).
 bs_status_t upload_tables(const SchedTables& tb, const WsLayout& layout, void* ws, cudaStream_t st);
 }  // namespace bs
@@ -49,6 +56,9 @@ inline SchedView make_sched_view(uint8_t* ws, const WsLayout& L, const SchedTabl
   sv.items = reinterpret_cast<const Item*>(ws + L.items_off);
   sv.spans = reinterpret_cast<const Span*>(ws + L.spans_off);
   sv.groups = reinterpret_cast<const Group*>(ws + L.groups_off);
+  sv.tmaps = reinterpret_cast<const CUtensorMap*>(ws + L.tmaps_off);
+  sv.n_span_clips = (int32_t)tb.clip_span_rows.size();
+  sv.n_item_clips = (int32_t)tb.clip_item_rows.size();
   sv.n_groups = (int32_t)tb.groups.size();
   sv.n_units = tb.n_units;
   sv.n_heads = n_heads;

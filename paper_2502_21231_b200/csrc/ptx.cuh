@@ -197,6 +197,15 @@ __device__ __forceinline__ void mbar_wait_warp(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap* m) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(m)) : "memory");
 }
+// A tensor map that lives in global memory (written by the host with a cudaMemcpy before the
+// launch - hence scope .sys - at an address that earlier launches used for other maps): make the
+// TMA unit read the current 128 bytes, not a copy its descriptor cache may still hold for that
+// address.  Executed by the thread that is going to use the map.
+__device__ __forceinline__ void tensormap_acquire(const CUtensorMap* m) {
+  asm volatile("fence.proxy.tensormap::generic.acquire.sys [%0], 128;" ::"l"(
+                   reinterpret_cast<uint64_t>(m))
+               : "memory");
+}
 // 3D tiled load: coordinates (c0 innermost, c1, c2) -> smem, completes tx bytes on `bar`
 __device__ __forceinline__ void tma_load_3d(void* smem_dst, const CUtensorMap* m, uint64_t* bar,
                                             int32_t c0, int32_t c1, int32_t c2) {

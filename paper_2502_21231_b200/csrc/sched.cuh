@@ -15,7 +15,10 @@ struct SchedView {  // device pointers into the uploaded workspace
   const Item* items;
   const Span* spans;
   const Group* groups;
+  const CUtensorMap* tmaps;  // clipped tensor maps of ragged range ends (worklist.h), 128-byte aligned
   int32_t n_groups, n_units, n_heads;
+  int32_t n_span_clips;      // bwd: the K / V maps of the item clips follow 2 * n_span_clips Q / dO maps
+  int32_t n_item_clips;
 };
 
 struct Unit {
@@ -129,6 +132,28 @@ struct UnitConsumerT {  // every consuming thread
       u->sp[1] = r->sp[slot][1];
     }
     ptx::mbar_arrive(&r->empty[slot]);
+    ++n;
+    return w >= 0;
+  }
+  // Warp-collective form for the lanes in `mask` (all of them call it, converged): lane `leader`
+  // alone polls the slot's barrier and releases the slot; the others park at the warp barrier.
+  // For roles that run far ahead of the pipeline and would otherwise have 32 lanes polling a
+  // barrier for the length of a unit - shared-memory polls that the tensor core's operand reads
+  // and the other warps of the scheduler partition pay for (measured: 5-9 % of either kernel).
+  __device__ __forceinline__ bool next_warp(Unit* u, uint32_t mask, int leader) {
+    const uint32_t slot = n % kSlots, ph = (n / kSlots) & 1;
+    const bool lead = (threadIdx.x & 31) == leader;
+    if (lead) ptx::mbar_wait(&r->full[slot], ph);
+    __syncwarp(mask);
+    const int32_t w = r->unit[slot];
+    if (w >= 0) {
+      u->item = r->item[slot];
+      u->head = r->head[slot];
+      u->sp[0] = r->sp[slot][0];
+      u->sp[1] = r->sp[slot][1];
+    }
+    __syncwarp(mask);
+    if (lead) ptx::mbar_arrive(&r->empty[slot]);
     ++n;
     return w >= 0;
   }

@@ -2,7 +2,12 @@
 #include "worklist.h"
 
 #include <algorithm>
+#include <map>
 #include <new>
+
+#ifndef BS_FWD_LONE_FIRST
+#define BS_FWD_LONE_FIRST 1  // experiment switch
+#endif
 
 namespace bs {
 
@@ -51,21 +56,37 @@ inline int32_t clamp_offset(int32_t off, int32_t q_len, int32_t k_len) {
 }
 }  // namespace
 
-WsLayout ws_layout(size_t n_items, size_t n_spans, size_t n_groups, size_t n_fill) {
+WsLayout ws_layout(size_t n_items, size_t n_spans, size_t n_groups, size_t n_fill, size_t tmap_bytes) {
   WsLayout L;
   L.items_off = sizeof(SchedHeader);
   L.spans_off = align256(L.items_off + n_items * sizeof(Item));
   L.groups_off = align256(L.spans_off + n_spans * sizeof(Span));
   L.fill_off = align256(L.groups_off + n_groups * sizeof(Group));
-  L.total = align256(L.fill_off + n_fill * sizeof(RowRange));
+  L.tmaps_off = align256(L.fill_off + n_fill * sizeof(RowRange));
+  L.total = align256(L.tmaps_off + tmap_bytes);
   return L;
 }
+
+namespace {
+// index of `end_row` in `rows` (appended if new); `seen` maps end row -> index
+int32_t clip_index(std::map<int32_t, int32_t>& seen, std::vector<int32_t>& rows, int32_t end_row) {
+  auto it = seen.find(end_row);
+  if (it != seen.end()) return it->second;
+  const int32_t idx = (int32_t)rows.size();
+  rows.push_back(end_row);
+  seen.emplace(end_row, idx);
+  return idx;
+}
+}  // namespace
 
 size_t ws_upper_bound(int64_t rows, int32_t n_segs, bool bwd) {
   // items: every distinct range of length L yields ceil(L / tile) <= L / tile + 1 items
   const int64_t tile = bwd ? kTile : 2 * kTile;
-  const size_t n_items = (size_t)(rows / tile + n_segs + 1);
-  return ws_layout(n_items, (size_t)n_segs, (size_t)n_segs, (size_t)n_segs + 1).total;
+  // forward: a range may add a lone first tile besides its last, partly filled item
+  const size_t n_items = (size_t)(rows / tile + (bwd ? 1 : 2) * (int64_t)n_segs + 1);
+  // clipped tensor maps: forward one (V) per key range; backward two per query range + two per key range
+  const size_t tmap_bytes = (size_t)n_segs * (bwd ? 4 : 1) * kTensorMapBytes;
+  return ws_layout(n_items, (size_t)n_segs, (size_t)n_segs, (size_t)n_segs + 1, tmap_bytes).total;
 }
 
 namespace {
@@ -123,6 +144,7 @@ bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
                                                 : segs[a].q_end < segs[b].q_end;
     });
     std::vector<Range> ranges;
+    std::map<int32_t, int32_t> seen_span;
     for (int32_t i = 0; i < n_segs;) {
       const bs_seg_t& g0 = segs[order[i]];
       int32_t j = i;
@@ -130,26 +152,31 @@ bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
       while (j < n_segs && segs[order[j]].q_begin == g0.q_begin &&
              segs[order[j]].q_end == g0.q_end) {
         const bs_seg_t& g = segs[order[j]];
-        out->spans.push_back({g.k_begin, g.k_end - g.k_begin,
-                              clamp_offset(g.causal_offset, g.q_end - g.q_begin, g.k_end - g.k_begin),
-                              0});
+        const int32_t k_len = g.k_end - g.k_begin;
+        out->spans.push_back({g.k_begin, k_len,
+                              clamp_offset(g.causal_offset, g.q_end - g.q_begin, k_len),
+                              k_len % kTile ? clip_index(seen_span, out->clip_span_rows, g.k_end) : -1});
         ++j;
       }
       ranges.push_back({g0.q_begin, g0.q_end});
       const int32_t q_len = g0.q_end - g0.q_begin;
-      group_items.push_back({(int32_t)out->items.size(), ceil_div(q_len, 2 * kTile)});
-      for (int32_t a0 = 0; a0 < q_len; a0 += 2 * kTile) {
+      const int32_t first_item = (int32_t)out->items.size();
+      // An item is two 128-row tiles that share the CTA (one TMEM slot each).  A range with an
+      // odd number of tiles leaves one tile alone, and a lone tile runs at half the CTA's rate
+      // for all of its key blocks: the lone one is the range's FIRST tile (the fewest visible
+      // blocks under a causal mask), not its last (the most).  `limit` bounds the item's rows.
+      auto emit = [&](int32_t a0, int32_t limit) {
         Item it{};
         it.row0 = g0.q_begin + a0;
         it.local0 = a0;
-        it.range_len = q_len;
+        it.range_len = limit;
         it.span_begin = span_begin;
         it.n_spans = j - i;
         int32_t cost = 0;
         for (int t = 0; t < 2; ++t) {
           const int32_t at = a0 + t * kTile;
-          if (at >= q_len) break;
-          const int64_t a_last = std::min<int64_t>(at + kTile, q_len) - 1;
+          if (at >= limit) break;
+          const int64_t a_last = std::min<int64_t>(at + kTile, limit) - 1;
           for (int32_t s = span_begin; s < span_begin + it.n_spans; ++s) {
             const int64_t vis = std::min<int64_t>(out->spans[s].len, a_last + out->spans[s].off + 1);
             if (vis > 0) it.tile_blocks[t] += (int32_t)ceil_div(vis, kTile);
@@ -158,7 +185,15 @@ bs_status_t build_fwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
         }
         it.cost = cost;
         out->items.push_back(it);
+      };
+      const int32_t n_tiles = ceil_div(q_len, kTile);
+      int32_t a0 = 0;
+      if (BS_FWD_LONE_FIRST && n_tiles > 1 && n_tiles % 2 == 1) {
+        emit(0, kTile);
+        a0 = kTile;
       }
+      for (; a0 < q_len; a0 += 2 * kTile) emit(a0, q_len);
+      group_items.push_back({first_item, (int32_t)out->items.size() - first_item});
       i = j;
     }
     bs_status_t rc = finish_groups(group_items, n_heads, out);
@@ -185,6 +220,7 @@ bs_status_t build_bwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
                                                 : segs[a].k_end < segs[b].k_end;
     });
     std::vector<Range> ranges;
+    std::map<int32_t, int32_t> seen_span, seen_item;
     for (int32_t i = 0; i < n_segs;) {
       const bs_seg_t& g0 = segs[order[i]];
       int32_t j = i;
@@ -192,9 +228,10 @@ bs_status_t build_bwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
       while (j < n_segs && segs[order[j]].k_begin == g0.k_begin &&
              segs[order[j]].k_end == g0.k_end) {
         const bs_seg_t& g = segs[order[j]];
-        out->spans.push_back({g.q_begin, g.q_end - g.q_begin,
-                              clamp_offset(g.causal_offset, g.q_end - g.q_begin, g.k_end - g.k_begin),
-                              0});
+        const int32_t q_len = g.q_end - g.q_begin;
+        out->spans.push_back({g.q_begin, q_len,
+                              clamp_offset(g.causal_offset, q_len, g.k_end - g.k_begin),
+                              q_len % kTile ? clip_index(seen_span, out->clip_span_rows, g.q_end) : -1});
         ++j;
       }
       ranges.push_back({g0.k_begin, g0.k_end});
@@ -207,6 +244,7 @@ bs_status_t build_bwd_tables(const bs_seg_t* segs, int32_t n_segs, int32_t q_row
         it.range_len = k_len;
         it.span_begin = span_begin;
         it.n_spans = j - i;
+        it.tile_blocks[0] = b0 + kTile > k_len ? clip_index(seen_item, out->clip_item_rows, g0.k_end) : -1;
         int32_t cost = 0;
         for (int32_t s = span_begin; s < span_begin + it.n_spans; ++s) {
           // query a sees key b0 iff a >= b0 - off: query tiles from floor(a_min / tile) on

@@ -11,6 +11,9 @@
 // Forward item  = up to 256 consecutive query rows (two 128-row MMA tiles) of one distinct query
 //                 range; its spans are the key ranges of every segment on that query range
 //                 (softmax over the union).  The kernel multiplies the item list by the Q heads.
+//                 A range with an odd number of tiles gives its FIRST tile an item of its own
+//                 (a lone tile runs at half the CTA's rate; under a causal mask the first tile
+//                 has the fewest key blocks), then pairs.
 // Backward item = one 128-key tile of one distinct key range; its spans are the query ranges of
 //                 every segment on that key range.  The kernel multiplies the list by the KV heads
 //                 and loops over the G query heads of the group and the visible query tiles.
@@ -23,21 +26,26 @@
 namespace bs {
 
 constexpr int kTile = 128;  // MMA tile edge in rows / keys
+constexpr size_t kTensorMapBytes = 128;  // sizeof(CUtensorMap)
 
 struct Span {     // forward: a key range;  backward: a query range
   int32_t begin;  // first row in the K/V (fwd) or Q (bwd) buffer
   int32_t len;    // rows
   int32_t off;    // key b visible to query a  iff  b <= a + off  (a, b local to their ranges)
-  int32_t pad;
+  int32_t clip;   // index of the range end's clipped tensor maps (SchedTables::clip_span_rows),
+                  // -1 if the range's length is a multiple of the tile (no ragged last tile)
 };
 struct Item {
   int32_t row0;        // first buffer row of the item (fwd: Q rows; bwd: K/V rows)
   int32_t local0;      // index of row0 inside its range (fwd: a0; bwd: b0)
-  int32_t range_len;   // length of the range the item belongs to (q_len fwd, k_len bwd)
+  int32_t range_len;   // bwd: length of the key range; fwd: end of the item's rows inside its query
+                       // range (the range length, or local0 + 128 for a lone first tile)
   int32_t span_begin;  // first span in the span table
   int32_t n_spans;
   int32_t cost;        // 128x128 blocks the item visits per head
-  int32_t tile_blocks[2];  // fwd: of those, the blocks of Q tile 0 / 1 (bwd: unused)
+  int32_t tile_blocks[2];  // fwd: of those, the blocks of Q tile 0 / 1; bwd: [0] = index of the
+                           // clipped K / V tensor maps (SchedTables::clip_item_rows) if this is the
+                           // ragged last tile of its key range, else -1
 };
 struct Group {           // the items of one distinct range; units = n_items x heads
   int32_t item_begin;    // first item in the item table
@@ -64,13 +72,22 @@ struct SchedTables {
   int32_t n_units = 0;         // sum over groups of n_items x heads
   std::vector<RowRange> fill;  // rows of the output range covered by no item
   int64_t max_fill_rows = 0;
+  // Range ends that are not tile-aligned: the ragged last tile of such a range is loaded through
+  // a tensor map whose row extent stops at the end, so that TMA zero-fills the rows past it
+  // (rows of another document, or uninitialised rows with NaN / Inf, never reach an MMA).
+  std::vector<int32_t> clip_span_rows;  // end rows of the spans' ranges (fwd: K/V rows, bwd: Q rows)
+  std::vector<int32_t> clip_item_rows;  // bwd: end rows of the key ranges (K/V rows)
+  std::vector<uint8_t> tmaps;           // 128-byte CUtensorMap objects, filled by the entry point:
+                                        // fwd [span clip] = V; bwd [2 i] = Q, [2 i + 1] = dO of
+                                        // span clip i, then [2 j] = K, [2 j + 1] = V of item clip j
 };
 
-// Workspace layout: [SchedHeader][items][spans][groups][fill ranges], each 256-byte aligned.
+// Workspace layout: [SchedHeader][items][spans][groups][fill ranges][tensor maps], each 256-byte
+// aligned.
 struct WsLayout {
-  size_t items_off, spans_off, groups_off, fill_off, total;
+  size_t items_off, spans_off, groups_off, fill_off, tmaps_off, total;
 };
-WsLayout ws_layout(size_t n_items, size_t n_spans, size_t n_groups, size_t n_fill);
+WsLayout ws_layout(size_t n_items, size_t n_spans, size_t n_groups, size_t n_fill, size_t tmap_bytes);
 // Upper bounds used by bs_attn_workspace_bytes (no segment list yet).
 size_t ws_upper_bound(int64_t rows, int32_t n_segs, bool bwd);
 

@@ -147,10 +147,13 @@ class DeviceRun:
             qs, qp, Qb = qs[rows], qp[rows], Qb[rows]
         return oracle.attn_fwd(Qb, self.kv3(Kb), self.kv3(Vb), qs, qp, ks, kp)
 
-    def oracle_backward(self):
+    def oracle_backward(self, LSE=None, delta=None):
+        """Plain definition over all keys (LSE = delta = None), or the same formulas under a given
+        normaliser LSE and a given delta ([Hq, q_rows] fp64): what a6 computes from ITS inputs."""
         opl, Kb, Vb, ks, kp = self.oracle_all_keys()
         dQ, dK, dV = oracle.attn_bwd(self.q3(self.Q_bits), self.kv3(Kb), self.kv3(Vb),
-                                     self.q3(self.dO_bits), opl["q_seq"], opl["q_pos"], ks, kp)
+                                     self.q3(self.dO_bits), opl["q_seq"], opl["q_pos"], ks, kp,
+                                     LSE=LSE, delta=delta)
         # split dK/dV back per step
         out, row = {}, 0
         for s in self.steps:
@@ -182,15 +185,23 @@ def o_compare(got_O, Oo, label=""):
     return float(diff.max())
 
 
-def grad_compare(name, got, want, block_of_row, label=""):
-    """One gradient tensor [rows, heads, D] against the oracle: relative L2 over the whole tensor
-    AND over every (document, head) block (a broken short document cannot hide behind a long
-    one), plus an element-wise bound.  Tolerance: BASELINE.json's 1e-2 relative L2, applied to
-    the whole tensor and to each block; a block whose oracle gradient is identically zero (a
-    length-1 document's dQ / dK) must be zero to 1e-4 rms.  Element-wise: the kernels round P and
-    dS to bf16 before the second MMAs, so an element's error is a random walk of relative steps
-    2^-9 over terms whose root-sum-square is of the order of the block's rms, plus the final bf16
-    rounding: |err| <= 2^-8 |want| + 0.06 rms(block)."""
+def grad_compare(name, got, want, block_of_row, label="", strict=True):
+    """One gradient tensor [rows, heads, D] against an oracle tensor: relative L2 over the whole
+    tensor (BASELINE.json: <= 1e-2) and - strict - over every block x head (block_of_row: e.g.
+    (ring step, document, 128-row chunk), so that a broken short document cannot hide behind a
+    long one), plus an element-wise bound.  A block whose oracle gradient is identically zero (a
+    length-1 document's dQ / dK) must be zero to 1e-4 rms.  Element-wise: P, dS and the result are
+    each rounded to bf16 (half an ulp: up to 2^-8 relative), so an element that one term dominates
+    may be off by 3 x 2^-8 of its value, and an element that many terms make up by a random walk
+    of such steps over terms whose root-sum-square is of the order of the block's rms:
+    |err| <= 3 x 2^-8 |want| + 0.08 rms(block).
+    strict=False (comparison with the PLAIN definition): only the whole-tensor bound is asserted
+    and the worst block is printed.  Why: delta = rowsum(dO o O) is formed from the bf16 output O
+    (as flash-attention backward does, and as a5 is defined), and dS = P (dP - delta) cancels when
+    one key dominates a row, so a two-token document's gradient can be smaller than the error
+    2^-9 |dO||O| that O's output rounding alone puts into delta.  The strict per-block and
+    element-wise bounds are therefore asserted against the oracle's formulas evaluated under the
+    LSE and delta the backward kernel was actually given (check_backward)."""
     got = np.asarray(got, np.float64)
     want = np.asarray(want, np.float64)
     assert got.shape == want.shape and got.ndim == 3
@@ -211,17 +222,28 @@ def grad_compare(name, got, want, block_of_row, label=""):
     worst = float(rel.max()) if rel.size else 0.0
     zero_rms = float(np.sqrt((num / np.maximum(cnt, 1))[zero]).max()) if zero.any() else 0.0
     rms = np.sqrt(den / np.maximum(cnt, 1))                     # [blocks, heads]
-    bound = 2.0 ** -8 * np.abs(want) + 0.06 * rms[blk][:, :, None] + 1e-6
+    # (absolute floor: fp32 cancellation noise where the oracle gradient is exactly zero, e.g. the
+    # first row of a document, whose dS = P (dP - delta) is 0 only in exact arithmetic)
+    bound = 3 * 2.0 ** -8 * np.abs(want) + 0.08 * rms[blk][:, :, None] + 1e-5
     ratio = float((np.abs(got - want) / bound).max()) if got.size else 0.0
-    print(f"{label}{name}: rel-L2 whole {whole:.2e}, worst (document, head) block {worst:.2e} over "
-          f"{int(live.sum())} x {H} blocks, zero-gradient blocks rms {zero_rms:.1e}, "
+    kind = "given LSE/delta" if strict else "plain definition"
+    print(f"{label}{name} vs {kind}: rel-L2 whole {whole:.2e}, worst block x head {worst:.2e} over "
+          f"{int(live.sum())} x {H}, zero-gradient blocks rms {zero_rms:.1e}, "
           f"element-wise err / bound max {ratio:.2f}")
-    assert whole <= TOL_GRAD, f"{label}{name} relative L2 error {whole}"
-    assert worst <= TOL_GRAD, (f"{label}{name} relative L2 error {worst} in (document, head) block "
-                               f"{np.unravel_index(int(rel.argmax()), rel.shape)}")
-    assert zero_rms <= 1e-4, f"{label}{name}: block with zero oracle gradient has rms {zero_rms}"
-    assert ratio <= 1.0, f"{label}{name}: element-wise error {ratio} x the bound"
+    assert whole <= TOL_GRAD, f"{label}{name} relative L2 error {whole} ({kind})"
+    if strict:
+        assert worst <= TOL_GRAD, (f"{label}{name} relative L2 error {worst} in block x head "
+                                   f"{np.unravel_index(int(rel.argmax()), rel.shape)}")
+        assert zero_rms <= 1e-4, f"{label}{name}: block with zero oracle gradient has rms {zero_rms}"
+        assert ratio <= 1.0, f"{label}{name}: element-wise error {ratio} x the bound"
     return whole
+
+
+def host_delta(O, dO_bits, rows, Hq, D):
+    """delta[h, i] = sum_d dO[i,h,d] * O[i,h,d] in fp64 from the bf16 O the device returned."""
+    o = oracle.bf16_to_f64(to_bits(O)).reshape(rows, Hq, D)
+    do = oracle.bf16_to_f64(dO_bits).reshape(rows, Hq, D)
+    return np.ascontiguousarray((o * do).sum(-1).T)
 
 
 def check_forward(run, O, LSE, rows=None, label=""):
@@ -255,23 +277,36 @@ def _blocks(step_idx, seq, n_seq):
     return ids
 
 
-def check_backward(run, dQ, grads, label=""):
-    """dQ, dK, dV of a DeviceRun against the oracle over all keys: whole tensor, every block of
-    (ring step, document, 128 buffer rows) x head, and element-wise (grad_compare).  Returns the
-    whole-tensor errors."""
-    dQo, go = run.oracle_backward()
+def check_backward(run, dQ, grads, O, LSE, label=""):
+    """dQ, dK, dV of a DeviceRun against the oracle over all keys.
+    (i) the plain definition: whole-tensor relative L2 (BASELINE.json's tolerance);
+    (ii) the same formulas under the LSE and delta = rowsum(dO o O) that bs_attn_bwd was given
+    (O, LSE: the forward's merged outputs, themselves checked by check_forward): whole tensor,
+    every (ring step, document, 128-row chunk) x head block, and element by element.
+    Returns the whole-tensor errors of (i)."""
     opl = oracle.oracle_plan(run.w.seqs)
     n_seq = len(run.w.seqs)
-    got = oracle.bf16_to_f64(to_bits(dQ)).reshape(dQo.shape)
-    errs = {"dQ": grad_compare("dQ", got, dQo, _blocks(0, opl["q_seq"], n_seq), label)}
+    qblk = _blocks(0, opl["q_seq"], n_seq)
     kblk, base = [], 0
     for s in run.steps:
         b = _blocks(0, opl["steps"][s]["k_seq"], n_seq) + base
         base = int(b.max()) + 1 if len(b) else base
         kblk.append(b)
     kblk = np.concatenate(kblk)
+    got_dQ = oracle.bf16_to_f64(to_bits(dQ)).reshape(run.q_rows, run.Hq, run.D)
+    got = {}
     for i, n in ((0, "dK"), (1, "dV")):
-        g = np.concatenate([oracle.bf16_to_f64(to_bits(grads[s][i])).reshape(go[s][i].shape)
-                            for s in run.steps])
-        errs[n] = grad_compare(n, g, np.concatenate([go[s][i] for s in run.steps]), kblk, label)
+        got[n] = np.concatenate([oracle.bf16_to_f64(to_bits(grads[s][i])).reshape(-1, run.Hkv, run.D)
+                                 for s in run.steps])
+    errs = {}
+    lse64 = LSE.double().cpu().numpy()
+    dl64 = host_delta(O, run.dO_bits, run.q_rows, run.Hq, run.D)
+    for strict, (dQo, go) in ((False, run.oracle_backward()),
+                              (True, run.oracle_backward(LSE=lse64, delta=dl64))):
+        e = {"dQ": grad_compare("dQ", got_dQ, dQo, qblk, label, strict)}
+        for i, n in ((0, "dK"), (1, "dV")):
+            e[n] = grad_compare(n, got[n], np.concatenate([go[s][i] for s in run.steps]), kblk,
+                                label, strict)
+        if not strict:
+            errs = e
     return errs

@@ -51,3 +51,27 @@ def test_single_process_passthrough():
     sys.path.insert(0, ROOT)
     from paper_2502_21231_b200 import dist_util as DU
     assert DU.max_over_ranks(None, [1.5, 2], "cpu") == [1.5, 2.0]
+
+
+def test_bench_gpus_2_starts_two_ranks():
+    """`python bench.py --gpus 2` with no launcher around it starts the two ranks itself
+    (torch.distributed.run on 127.0.0.1); here with --impl plumbing: the launch path, barrier and
+    max-over-ranks of the real bench on CPU/gloo, a host-only step in place of the device work."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items()
+           if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "3",
+                        "--warmup", "1", "--impl", "plumbing"], capture_output=True, text=True,
+                       timeout=300, env=env, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(x) for x in r.stdout.splitlines() if x.startswith("{")]
+    assert len(lines) == 1, r.stdout          # rank 0 alone prints
+    out = lines[0]
+    assert out["n_gpus"] == 2 and out["steps"] == 3 and out["impl"] == "plumbing"
+    assert out["value"] > 0 and out["q_rows"] == 32768
+    # one process, no launcher, one GPU asked for: no spawn
+    r1 = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "2", "--warmup", "1",
+                         "--impl", "plumbing"], capture_output=True, text=True, timeout=300, env=env,
+                        cwd=ROOT)
+    assert r1.returncode == 0 and json.loads(r1.stdout.strip().splitlines()[-1])["n_gpus"] == 1

@@ -212,12 +212,14 @@ def test_nan_in_rows_no_segment_covers(nprng, Hq, Hkv, D):
     q_pos = np.concatenate([np.arange(b - a, dtype=np.int32) for a, b in docs])
     cat = lambda xs: np.concatenate(xs)  # noqa: E731
     Oo, Lo = oracle.attn_fwd(cat(Qb), cat(Kb), cat(Vb), q_seq, q_pos, q_seq, q_pos)
-    dQo, dKo, dVo = oracle.attn_bwd(cat(Qb), cat(Kb), cat(Vb), cat(dOb), q_seq, q_pos, q_seq, q_pos)
     O, LSE, dQ, dK, dV = outs["nan"]
     rows = torch.cat([torch.arange(a, b) for a, b in docs]).cuda()
     f64 = lambda t, H: oracle.bf16_to_f64(U.to_bits(t[rows].contiguous())).reshape(len(rows), H, D)  # noqa: E731
-    U.o_compare(f64(O, Hq), Oo, "NaN-padded buffers: ")
-    assert np.abs(LSE[:, rows].double().cpu().numpy() - Lo).max() <= U.TOL_LSE
-    U.grad_compare("dQ", f64(dQ, Hq), dQo, q_seq, "NaN-padded buffers: ")
-    U.grad_compare("dK", f64(dK, Hkv), dKo, q_seq, "NaN-padded buffers: ")
-    U.grad_compare("dV", f64(dV, Hkv), dVo, q_seq, "NaN-padded buffers: ")
+    got_O, got_L = f64(O, Hq), LSE[:, rows].double().cpu().numpy()
+    U.o_compare(got_O, Oo, "NaN-padded buffers: ")
+    assert np.abs(got_L - Lo).max() <= U.TOL_LSE
+    dl = np.ascontiguousarray((got_O * oracle.bf16_to_f64(cat(dOb))).sum(-1).T)
+    for strict, kw in ((False, {}), (True, dict(LSE=got_L, delta=dl))):
+        ref = oracle.attn_bwd(cat(Qb), cat(Kb), cat(Vb), cat(dOb), q_seq, q_pos, q_seq, q_pos, **kw)
+        for name, g, want in zip(("dQ", "dK", "dV"), (f64(dQ, Hq), f64(dK, Hkv), f64(dV, Hkv)), ref):
+            U.grad_compare(name, g, want, q_seq, "NaN-padded buffers: ", strict)

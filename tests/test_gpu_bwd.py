@@ -17,7 +17,7 @@ def _run(w, fused_clear=False):
     O, LSE, _ = run.forward()
     U.check_forward(run, O, LSE, label=f"{w.name}: ")
     dQ, grads, _ = run.backward(O, LSE)
-    return U.check_backward(run, dQ, grads, label=f"{w.name}: ")
+    return U.check_backward(run, dQ, grads, O, LSE, label=f"{w.name}: ")
 
 
 @pytest.mark.parametrize("lens,Hq,Hkv,D", [

@@ -11,7 +11,8 @@ A full fp64 oracle pass is hours at these sizes, so the comparis
   * sparse-dO run: the backward again, same launches, with dO non-zero only on
     a sampled row set R.  Then dK and dV of EVERY key row (and dQ of R) are exactly what the
     oracle computes from the rows of R alone, at cost |R| x keys: every element of dK / dV of
-    every KV head is compared, per 128-key tile of every ring step, and dQ outside R must be 0;
+    every KV head is compared, per 128-key tile of every ring step, and dQ outside R must be 0
+    (oracle formulas under the LSE and delta the kernel was given, see gpu_util.grad_compare);
   * dense dO: dK, dV of every key row through the O(T) identities that hold for any set of query
     rows (softmax rows sum to 1, softmax shift invariance):
         sum_j dV[j,g,:] = sum_{h in g} sum_i dO[i,h,:]        sum_j dK[j,g,:] = 0      per sequence
@@ -149,19 +150,23 @@ def _check_sampled_rows(fr, dQ, n_random, n_boundary):
     Vall = np.concatenate(fr.Vb).reshape(-1, Hkv, D)
     qs, qp = fr.opl["q_seq"][rows], fr.opl["q_pos"][rows]
     Qs, dOs = fr.Qb.reshape(rows_q, Hq, D)[rows], fr.dOb.reshape(rows_q, Hq, D)[rows]
-    Oo, Lo = oracle.attn_fwd(Qs, Kall, Vall, qs, qp, ks, kp)
-    dQo, _, _ = oracle.attn_bwd(Qs, Kall, Vall, dOs, qs, qp, ks, kp)
-    del Kall, Vall
     ridx = torch.from_numpy(rows).cuda()
     got_O = fr.bits_of(fr.O[ridx]).reshape(len(rows), Hq, D)
     got_L = fr.LSE[:, ridx].double().cpu().numpy()
     got_dQ = fr.bits_of(dQ[ridx]).reshape(len(rows), Hq, D)
+    Oo, Lo = oracle.attn_fwd(Qs, Kall, Vall, qs, qp, ks, kp)
+    dQo, _, _ = oracle.attn_bwd(Qs, Kall, Vall, dOs, qs, qp, ks, kp)
+    # the same rows under the LSE and delta the backward kernel was given (gpu_util.grad_compare)
+    dl = np.ascontiguousarray((got_O * oracle.bf16_to_f64(dOs)).sum(-1).T)
+    dQi, _, _ = oracle.attn_bwd(Qs, Kall, Vall, dOs, qs, qp, ks, kp, LSE=got_L, delta=dl)
+    del Kall, Vall
     label = f"cfg{cfg} ({len(rows)} sampled rows): "
     U.o_compare(got_O, Oo, label)
     err_L = float(np.abs(got_L - Lo).max())
     assert err_L <= U.TOL_LSE, f"cfg{cfg}: LSE abs err {err_L}"
     # every sampled row is its own block: dQ of a row depends on that row only
-    U.grad_compare("dQ", got_dQ, dQo, np.arange(len(rows)), label)
+    U.grad_compare("dQ", got_dQ, dQo, np.arange(len(rows)), label, strict=False)
+    U.grad_compare("dQ", got_dQ, dQi, np.arange(len(rows)), label, strict=True)
     print(f"{label}LSE abs err {err_L:.1e}")
 
 
@@ -215,11 +220,17 @@ def _check_sparse_dO(fr, n_random, n_boundary):
     qs, qp = fr.opl["q_seq"][R], fr.opl["q_pos"][R]
     Q3, dO3 = fr.Qb.reshape(rows_q, Hq, D)[R], fr.dOb.reshape(rows_q, Hq, D)[R]
     got_dQ = fr.bits_of(dQ[ridx]).reshape(len(R), Hq, D)
+    # the oracle's formulas under the LSE and delta = rowsum(dO o O) the kernel was given for the
+    # rows of R (gpu_util.grad_compare says why); O and LSE themselves are checked on sampled rows
+    lse_R = fr.LSE[:, ridx].double().cpu().numpy()
+    dl_R = (fr.bits_of(fr.O[ridx]).reshape(len(R), Hq, D) * oracle.bf16_to_f64(dO3)).sum(-1).T
     for g in range(Hkv):
         hs = slice(g * G, (g + 1) * G)
         Kg, Vg = fr.kv_heads(fr.Kb, [g]), fr.kv_heads(fr.Vb, [g])
         dQo, dKo, dVo = oracle.attn_bwd(np.ascontiguousarray(Q3[:, hs]), Kg, Vg,
-                                        np.ascontiguousarray(dO3[:, hs]), qs, qp, ks, kp)
+                                        np.ascontiguousarray(dO3[:, hs]), qs, qp, ks, kp,
+                                        LSE=np.ascontiguousarray(lse_R[hs]),
+                                        delta=np.ascontiguousarray(dl_R[hs]))
         label = f"cfg{cfg} sparse dO ({len(R)} rows), KV head {g}: "
         U.grad_compare("dQ", got_dQ[:, hs], dQo, np.arange(len(R)), label)
         gk = np.concatenate([fr.bits_of(d[:, g]).reshape(-1, 1, D) for d in dKs])
@@ -241,18 +252,22 @@ def test_cfg2_full_size():
     qs, qp = fr.opl["q_seq"], fr.opl["q_pos"]
     pick = lambda bits: np.ascontiguousarray(bits.reshape(rows, fr.Hq, D)[:, heads])  # noqa: E731
     Qh, dOh, Kh, Vh = pick(fr.Qb), pick(fr.dOb), pick(fr.Kb[0]), pick(fr.Vb[0])
-    Oo, Lo = oracle.attn_fwd(Qh, Kh, Vh, qs, qp, qs, qp)
-    dQo, dKo, dVo = oracle.attn_bwd(Qh, Kh, Vh, dOh, qs, qp, qs, qp)
     hidx = torch.tensor(heads, device="cuda")
     label = f"cfg2 heads {heads}, all {rows} rows: "
-    U.o_compare(fr.bits_of(fr.O[:, hidx]).reshape(rows, len(heads), D), Oo, label)
-    err_L = float(np.abs(fr.LSE[hidx].double().cpu().numpy() - Lo).max())
+    got_O = fr.bits_of(fr.O[:, hidx]).reshape(rows, len(heads), D)
+    got_L = fr.LSE[hidx].double().cpu().numpy()
+    Oo, Lo = oracle.attn_fwd(Qh, Kh, Vh, qs, qp, qs, qp)
+    U.o_compare(got_O, Oo, label)
+    err_L = float(np.abs(got_L - Lo).max())
     assert err_L <= U.TOL_LSE, f"cfg2: LSE abs err {err_L}"
-    blk = U._blocks(0, qs, len(fr.w.seqs))
-    U.grad_compare("dQ", fr.bits_of(dQ[:, hidx]).reshape(rows, len(heads), D), dQo, blk, label)
-    U.grad_compare("dK", fr.bits_of(dKs[0][:, hidx]).reshape(rows, len(heads), D), dKo, blk, label)
-    U.grad_compare("dV", fr.bits_of(dVs[0][:, hidx]).reshape(rows, len(heads), D), dVo, blk, label)
     print(f"{label}LSE abs err {err_L:.1e}")
+    blk = U._blocks(0, qs, len(fr.w.seqs))
+    got = [fr.bits_of(t[:, hidx]).reshape(rows, len(heads), D) for t in (dQ, dKs[0], dVs[0])]
+    dl = np.ascontiguousarray((got_O * oracle.bf16_to_f64(dOh)).sum(-1).T)
+    for strict, ref in ((False, oracle.attn_bwd(Qh, Kh, Vh, dOh, qs, qp, qs, qp)),
+                        (True, oracle.attn_bwd(Qh, Kh, Vh, dOh, qs, qp, qs, qp, LSE=got_L, delta=dl))):
+        for name, g, want in zip(("dQ", "dK", "dV"), got, ref):
+            U.grad_compare(name, g, want, blk, label, strict)
 
 
 def test_cfg3_full_size():
