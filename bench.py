@@ -391,7 +391,9 @@ def run_ours(args, rank, world, local_rank):
                                        if pk["tflops_sustained"] else None,
                                        "frac_of_burst_peak": round(sus / world / pk["tflops"], 4),
                                        "sm_mhz_median": sampler.median_between(t_sus0, t_sus1)},
-                         "merge_gbs": {k: v for k, v in merge["by_config"].items()}},
+                         "merge_gbs": {k: {"gbs": v["gbs"], "of_n_to_1_probe": v["frac_of_n_to_1_probe"],
+                                               "of_measured_copy": v["frac_of_measured_copy"]}
+                                           for k, v in merge["by_config"].items()}},
             "cpu_baseline": {"value": fl / dt / 1e12, "unit": "TFLOP/s", "cores": thr, "kind": "oracle",
                              "sample": f"{CPU_BASELINE_HEADS} of {Hq} heads of {WORKLOAD}, all "
                                        f"{rows} tokens, fwd+bwd, fp64, {dt:.1f} s"},
@@ -437,13 +439,15 @@ def bench_merge(B, torch, pk):
         ms_alias = timed(lambda: B.lse_merge(Os, Ls, sh, (0, rows), Os[0], Ls[0]), 10 if n < 64 else 4)
         nbytes = (n + 1) * rows * Hq * (2 * D + 4)
         ms_n1 = timed(lambda: B.hbm_probe(Os, O, sink), 10 if n < 64 else 4)
-        ms_rd = timed(lambda: B.hbm_probe(Os + [O], None, sink), 10 if n < 64 else 4)
+        rd = (Os + [O])[:B.BS_MAX_MERGE_PARTS]          # n + 1 streams, at most 64
+        ms_rd = timed(lambda: B.hbm_probe(rd, None, sink), 10 if n < 64 else 4)
         pbytes = (n + 1) * rows * Hq * 2 * D
+        rbytes = len(rd) * rows * Hq * 2 * D
         gbs = nbytes / ms / 1e6
         out[f"cfg{cfg}"] = {"n_parts": n, "rows": rows, "heads": Hq, "ms": round(ms, 4), "bytes": nbytes,
                             "gbs": round(gbs, 1), "gbs_output_aliases_part0": round(nbytes / ms_alias / 1e6, 1),
                             "probe_n_to_1_gbs": round(pbytes / ms_n1 / 1e6, 1),
-                            "probe_pure_read_gbs": round(pbytes / ms_rd / 1e6, 1),
+                            "probe_pure_read_gbs": round(rbytes / ms_rd / 1e6, 1),
                             "frac_of_n_to_1_probe": round(gbs / (pbytes / ms_n1 / 1e6), 4),
                             "frac_of_measured_copy": round(gbs / pk["hbm"], 4),
                             "frac_of_nominal_8000": round(gbs / 8000.0, 4)}

@@ -57,9 +57,6 @@ constexpr float kRescaleThreshold = 8.f;  // log2 units
 #define BS_FWD_EMU 1
 #endif
 constexpr int kEmuOf4 = BS_FWD_EMU;  // of every 4 column pairs, this many take the FMA-pipe exp2
-#ifndef BS_FWD_LASTLOCK
-#define BS_FWD_LASTLOCK 1  // 0: a unit's last PV chunk (no S MMA behind it) is issued without the turn lock
-#endif
 
 struct FwdParams {
   SchedView sv;     // units = query items x n_q_heads
@@ -416,9 +413,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
           // The batch [PV_t(b), S_t(b+1)] is issued under the turn lock: batches of the two tiles
           // enter the tensor pipe whole, one after the other, which keeps the tiles half a period
           // apart (softmax of one under the MMAs of the other) instead of drifting into phase.
-          const bool locked = BS_FWD_LASTLOCK || has_next;  // (experiment switch)
-          if (locked)
-            while (atom_cas_shared(turn, 0u, 1u) != 0u) __nanosleep(20);
+          while (atom_cas_shared(turn, 0u, 1u) != 0u) __nanosleep(20);
           if (lane == 0) TRACE(2 + t, 1, tr_it);
           if (cur.active(t)) {
             {
@@ -433,7 +428,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             release(k_stage);
           }
           if (lane == 0) TRACE(2 + t, 3, tr_it);
-          if (locked) st_release_shared(turn, 0u);
+          st_release_shared(turn, 0u);
           if (lane == 0) TRACE(2 + t, 4, tr_it);
           ++tr_it;
           if (!has_next) break;

@@ -156,6 +156,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     if (++spins > (1u << 26)) {  // try_wait itself sleeps up to a HW time limit per poll
       printf("bs: mbarrier wait timed out (block %d thread %d bar %u parity %u)\n", blockIdx.x,
              threadIdx.x, smem_u32(bar), parity);
+#ifdef BS_DEBUG_TIMEOUT  // debug builds: let the other stuck threads report before the trap
+      for (int i = 0; i < 200; ++i) __nanosleep(1000000);
+#endif
       __trap();
     }
   }

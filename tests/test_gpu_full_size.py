@@ -201,7 +201,7 @@ def _check_identities(fr, dQ, dKs, dVs):
     assert e_qk <= 1e-2, f"cfg{cfg}: Q.dQ = K.dK identity off by {e_qk}"
 
 
-def _check_sparse_dO(fr, n_random, n_boundary):
+def _check_sparse_dO(fr, n_random, n_boundary, groups=None):
     """dO non-zero on a sampled row set R only; every dK / dV element of every
     ring step, and dQ of R, against the oracle evaluated on the rows of R over all keys."""
     U, cfg, Hq, Hkv, D, rows_q = fr.U, fr.cfg, fr.Hq, fr.Hkv, fr.D, fr.rows_q
@@ -224,7 +224,7 @@ def _check_sparse_dO(fr, n_random, n_boundary):
     # rows of R (gpu_util.grad_compare says why); O and LSE themselves are checked on sampled rows
     lse_R = fr.LSE[:, ridx].double().cpu().numpy()
     dl_R = (fr.bits_of(fr.O[ridx]).reshape(len(R), Hq, D) * oracle.bf16_to_f64(dO3)).sum(-1).T
-    for g in range(Hkv):
+    for g in (range(Hkv) if groups is None else groups):
         hs = slice(g * G, (g + 1) * G)
         Kg, Vg = fr.kv_heads(fr.Kb, [g]), fr.kv_heads(fr.Vb, [g])
         dQo, dKo, dVo = oracle.attn_bwd(np.ascontiguousarray(Q3[:, hs]), Kg, Vg,
@@ -295,4 +295,6 @@ def test_cfg5_full_size():
     _check_sampled_rows(fr, dQ, 1, 3)  # ~1e11 fp64 flop of oracle per sampled row at 2M keys
     _check_identities(fr, dQ, dKs, dVs)
     del dQ, dKs, dVs
-    _check_sparse_dO(fr, 8, 4)
+    # two of the eight KV groups (the oracle pass over 2M keys costs ~25 s per group; the other
+    # groups' dK / dV are covered by the identities above and, element-wise, by the twins)
+    _check_sparse_dO(fr, 8, 6, groups=(0, 5))
