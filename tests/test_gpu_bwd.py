@@ -56,7 +56,8 @@ def test_twin_of_cfg4_every_rank(r, ragged):
 @pytest.mark.parametrize("ragged", [False, True], ids=["c256", "ragged"])
 @pytest.mark.parametrize("r", [0, 31, 32, 63])
 def test_twin_of_cfg5_ranks(r, ragged):
-    print(_run(workloads.scaled_twin(5, 256, ragged, rank=r, kv_heads=2)))
+    # (one KV group of 6 query heads: the oracle pass over 32768 keys stays at ~6 s per case)
+    print(_run(workloads.scaled_twin(5, 256, ragged, rank=r, kv_heads=1)))
 
 
 def test_twin_of_cfg3_all_eight_groups():
