@@ -5,7 +5,7 @@
 //   warps 0-3   compute warpgroup A: query columns  0..63  of the transposed 128x128 tile
 //   warps 4-7   compute warpgroup B: query columns 64..127
 //   warp  8     MMA issuer (under elect_one: uniform-register descriptors, back-to-back UTCHMMA)
-//   warp  9     TMA producer       warp 10  scheduler (sched.cuh)       warp 11  LSE / delta staging
+//   warp  9     TMA producer (+ LSE/delta staging)       warp 10  scheduler (sched.cuh)
 //   warps 12-15 dQ drain warpgroup: TMEM -> registers -> shared -> TMA reduce-add into dQ_acc
 // A unit is (one 128-key tile of a key range, one KV head).  The CTA keeps dK and dV of the tile
 // in TMEM and loops over the G query heads of the group and over every 128-row query tile that
@@ -55,10 +55,6 @@ using UnitConsumer = UnitConsumerT<kBwdSchedSlots>;
 constexpr int kSchedRingBytes = SchedRing::kBytes;
 
 constexpr int kBwdThreads = 512;   // 2 compute WGs, auxiliary WG (MMA, TMA, scheduler), dQ drain WG
-#ifndef BS_BWD_STAGE_WARP
-#define BS_BWD_STAGE_WARP 1  // 1: the otherwise idle warp 11 stages LSE / delta; 0: the TMA warp does
-#endif
-constexpr bool kStageWarp11 = BS_BWD_STAGE_WARP != 0;
 #ifndef BS_BWD_REGS_C
 #define BS_BWD_REGS_C 144
 #define BS_BWD_REGS_A 64
@@ -241,8 +237,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     __trap();
   }
   if (warp == 9 && lane == 0) {
-    // consumers: compute threads, MMA lane, TMA lane (, staging warp's lane), drain warpgroup
-    sched_ring_init(sched, kComputeThreads + 2 + (kStageWarp11 ? 1 : 0) + kTile);
+    sched_ring_init(sched, kComputeThreads + 2 + kTile);  // compute + MMA lane + TMA lane + drain WG
     mbar_init(k_full, 1);
     mbar_init(k_empty, 1);
     mbar_init(v_full, 1);
@@ -351,18 +346,16 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tma_load_3d(smem + L::kQOff + st * L::kTileBytes + half * (kTile * 128), mQ,
                         &q_full[st], half * 64, h, qrow);
         }
-        if (!kStageWarp11) {
-          // -lse*log2e (-inf for rows outside the query range) and -delta*scale
-          for (int c = lane; c < kTile; c += 32) {
-            const int a = wk.qi * kTile + c;
-            const bool ok = a < wk.sp.len;
-            const int64_t idx = (int64_t)h * p.lse_head_stride + qrow + c;
-            // negated, so that the compute warps fold them in with one packed FMA each
-            lse_s[st * kTile + c] = ok ? -p.LSE[idx] * 1.4426950408889634f : -CUDART_INF_F;
-            delta_s[st * kTile + c] = ok ? -p.delta[idx] * p.scale : 0.f;
-          }
-          mbar_arrive(&q_full[st]);
+        // -lse*log2e (-inf for rows outside the query range) and -delta*scale
+        for (int c = lane; c < kTile; c += 32) {
+          const int a = wk.qi * kTile + c;
+          const bool ok = a < wk.sp.len;
+          const int64_t idx = (int64_t)h * p.lse_head_stride + qrow + c;
+          // negated, so that the compute warps fold them in with one packed FMA each
+          lse_s[st * kTile + c] = ok ? -p.LSE[idx] * 1.4426950408889634f : -CUDART_INF_F;
+          delta_s[st * kTile + c] = ok ? -p.delta[idx] * p.scale : 0.f;
         }
+        mbar_arrive(&q_full[st]);
         if (lane == own_q) {
           mbar_wait(do_empty, (it_n & 1) ^ 1);
           mbar_arrive_expect_tx(do_full, L::kTileBytes);
@@ -377,42 +370,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         __syncwarp();
       }
       ++item_n;
-    }
-  } else if (kStageWarp11 && warp == 11) {
-    // ================================== LSE / delta staging ==================================
-    // -lse*log2e and -delta*scale of an iteration's 128 query rows, from global memory into the
-    // stage's shared-memory slots (the 32 arrivals of q_full[stage] besides the TMA's).  On the
-    // TMA warp these dependent global loads (~800-1000 cycles) sat between the request of Q(n+1)
-    // and the wait for dO's buffer, so that dO(n+1) - single-buffered, its load on the
-    // iteration's critical path - was requested late whenever its buffer came free meanwhile.
-    // Here the values are fetched into registers BEFORE the wait for the stage.
-    uint32_t it_n = 0;
-    UnitConsumer cons{sched};
-    Unit u;
-    while (cons.next_warp(&u, 0xffffffffu, 0)) {
-      const int g = u.head;
-      BwdWalker wk;
-      wk.init(p.sv.spans, u, p.group);
-      for (; !wk.done(); wk.next(), ++it_n) {
-        const int st = it_n & 1, h = g * p.group + wk.hi, qrow = wk.q_row();
-        float nl[kTile / 32], nd[kTile / 32];
-#pragma unroll
-        for (int k = 0; k < kTile / 32; ++k) {
-          const int c = lane + 32 * k;
-          const bool ok = wk.qi * kTile + c < wk.sp.len;
-          const int64_t idx = (int64_t)h * p.lse_head_stride + qrow + c;
-          // negated, so that the compute warps fold them in with one packed FMA each
-          nl[k] = ok ? -p.LSE[idx] * 1.4426950408889634f : -CUDART_INF_F;
-          nd[k] = ok ? -p.delta[idx] * p.scale : 0.f;
-        }
-        mbar_wait_warp(&q_empty[st], ((it_n >> 1) & 1) ^ 1);  // one lane polls
-#pragma unroll
-        for (int k = 0; k < kTile / 32; ++k) {
-          lse_s[st * kTile + lane + 32 * k] = nl[k];
-          delta_s[st * kTile + lane + 32 * k] = nd[k];
-        }
-        mbar_arrive(&q_full[st]);
-      }
     }
   } else if (warp == 10) {
     // ======================================== scheduler ========================================
