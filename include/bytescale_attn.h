@@ -262,6 +262,32 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
                         int32_t out_row_end, void* O, float* LSE, void* ws, size_t ws_bytes,
                         void* stream, float* dQ_acc_clear);
 
+/* bs_attn_fwd for callers that may not allocate device memory (a CUDA graph being captured, a
+ * serving loop, a harness that forbids cudaMalloc): the same operation, arguments, kernels and
+ * results as bs_attn_fwd, but the work-item tables, the scheduler's cursor and the
+ * clipped tensor maps live in a scratch array INSIDE the library (static __device__,
+ * BS_ATTN_STATIC_SCRATCH_BYTES per GPU that loads the library, held until the process exits)
+ * instead of a caller workspace.  The call allocates nothing on the device or in pinned memory
+ * (no cudaMalloc / cudaFree / cudaHostAlloc, no allocating library routine; host heap only for
+ * the work list): the tables reach the scratch as kernel PARAMETERS of small copy kernels
+ * (3584 bytes per launch), so nothing is read from host memory after the call returns and the
+ * host never waits for the stream.
+ *   Limit: the call's tables must fit the array.  A call fits whenever
+ * bs_attn_workspace_bytes(shape, n_segs, 0, &b) gives b <= BS_ATTN_STATIC_SCRATCH_BYTES (an
+ * upper bound; the exact size is checked); otherwise BS_ERR_WORKSPACE with both sizes in
+ * bs_last_error(), before anything is enqueued - use bs_attn_fwd then.  256 KiB holds e.g. a
+ * 131072-row packed buffer of ~1000 ragged documents.
+ *   Sharing: every call on a device uses the SAME array.  Each call rewrites all of it that it
+ * reads (cursor included), so the previous call's contents never matter, but two calls whose
+ * kernels can overlap on the GPU (different streams without an ordering, or host threads on
+ * different streams) race on it: keep all bs_attn_fwd_static calls of a device on one stream or
+ * order them with events.  Other errors and all argument rules as bs_attn_fwd. */
+#define BS_ATTN_STATIC_SCRATCH_BYTES 262144
+bs_status_t bs_attn_fwd_static(const bs_attn_shape_t* shape, const void* Q, const void* K,
+                               const void* V, const bs_seg_t* segs, int32_t n_segs,
+                               int32_t out_row_begin, int32_t out_row_end, void* O, float* LSE,
+                               void* stream, float* dQ_acc_clear);
+
 /* Backward preparation (a5): delta[h,i] = sum_d dO[i,h,d] * O_final[i,h,d] for all q_rows, and
  * dQ_acc = 0 (skipped if dQ_acc is NULL: the accumulator was cleared by bs_attn_fwd).  O_final is
  * the MERGED output.  All device pointers. */

@@ -112,6 +112,8 @@ lib.bs_balance_destroy.argtypes = [_vp]
 lib.bs_attn_workspace_bytes.argtypes = [_P(Shape), _i32, ctypes.c_int, _P(_sz)]
 lib.bs_attn_fwd.argtypes = [_P(Shape), _vp, _vp, _vp, _P(Seg), _i32, _i32, _i32, _vp, _vp, _vp,
                             _sz, _vp, _vp]
+lib.bs_attn_fwd_static.argtypes = [_P(Shape), _vp, _vp, _vp, _P(Seg), _i32, _i32, _i32, _vp, _vp,
+                                   _vp, _vp]
 lib.bs_attn_bwd_prep.argtypes = [_P(Shape), _vp, _vp, _vp, _vp, _vp]
 lib.bs_attn_bwd.argtypes = [_P(Shape), _vp, _vp, _vp, _vp, _vp, _vp, _P(Seg), _i32, _vp, _vp, _vp,
                             _vp, _sz, _vp]
@@ -131,7 +133,7 @@ EXPORTS = ["bs_status_string", "bs_last_error", "bs_version", "bs_plan", "bs_pla
            "bs_balance_exec_times", "bs_balance_makespan", "bs_balance_n_microbatches",
            "bs_balance_microbatch", "bs_balance_destroy", "bs_attn_workspace_bytes", "bs_attn_fwd",
            "bs_attn_bwd_prep", "bs_attn_bwd", "bs_attn_bwd_finish", "bs_lse_merge", "bs_softmax_xent",
-           "bs_hbm_probe",
+           "bs_hbm_probe", "bs_attn_fwd_static",
            "bs_launch_count", "bs_launch_count_reset"]
 
 
@@ -264,6 +266,18 @@ def attn_fwd(shape, Q, K, V, segs, out_rows, O, LSE, ws, dQ_acc_clear=None):
                            out_rows[1], _ptr(O), _ptr(LSE), _ptr(ws), ws.numel() * ws.element_size(),
                            _stream(), None if dQ_acc_clear is None else _ptr(dQ_acc_clear)),
            "bs_attn_fwd")
+
+
+STATIC_SCRATCH_BYTES = 262144  # BS_ATTN_STATIC_SCRATCH_BYTES
+
+
+def attn_fwd_static(shape, Q, K, V, segs, out_rows, O, LSE, dQ_acc_clear=None):
+    """bs_attn_fwd_static: bs_attn_fwd without a caller workspace (library-owned static scratch)."""
+    sarr, n = make_segs(segs)
+    _check(lib.bs_attn_fwd_static(ctypes.byref(shape), _ptr(Q), _ptr(K), _ptr(V), sarr, n,
+                                  out_rows[0], out_rows[1], _ptr(O), _ptr(LSE), _stream(),
+                                  None if dQ_acc_clear is None else _ptr(dQ_acc_clear)),
+           "bs_attn_fwd_static")
 
 
 def attn_bwd_prep(shape, O_final, dO, delta, dQ_acc):

@@ -783,3 +783,195 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// bs_attn_fwd_static — the forward for callers that may not allocate (include/bytescale_attn.h).
+// Same kernels and results as bs_attn_fwd; what differs is where the scratch lives (the array
+// below instead of a caller workspace) and how the tables get there (kernel parameters of a copy
+// kernel instead of a DMA from the library's pinned ring, which is allocated lazily).
+// ------------------------------------------------------------------------------------------------
+#include <cstring>
+#include <mutex>
+#include <new>
+#include <vector>
+
+namespace {
+
+constexpr size_t kStaticScratchBytes = BS_ATTN_STATIC_SCRATCH_BYTES;
+// Held by every GPU that loads this library, until the process exits.  In HOST code this name is
+// a host-side stand-in, not a device address: kernels get the address cudaGetSymbolAddress
+// returns (static_scratch_address below), never `g_static_scratch` itself.
+static __device__ __align__(256) uint8_t g_static_scratch[kStaticScratchBytes];
+
+constexpr int kChunkBytes = 3584;  // per launch; the classic 4 KB parameter space minus the rest
+struct TableChunk {
+  uint4 v[kChunkBytes / 16];
+};
+static_assert(sizeof(TableChunk) == kChunkBytes && kChunkBytes % 256 == 0, "chunk size");
+
+// dst[0 .. n_vec) = the chunk.  The tables include tensor maps, which the forward's TMA warp reads
+// through the tensormap proxy after its own acquire fence; the release half goes here.
+__global__ void __launch_bounds__(kChunkBytes / 16)
+static_scratch_upload_kernel(const __grid_constant__ TableChunk c, uint4* dst, int n_vec) {
+  const int i = threadIdx.x;
+  if (i < n_vec) dst[i] = c.v[i];
+  __threadfence();
+  asm volatile("fence.proxy.tensormap::generic.release.gpu;" ::: "memory");
+}
+
+constexpr int kMaxScratchDevices = 64;
+std::mutex g_scratch_mu;
+uint8_t* g_scratch_addr[kMaxScratchDevices];  // device address of g_static_scratch, per device
+
+// Set-up, once per device, with that device current.
+bs_status_t static_scratch_address(uint8_t** out) {
+  int dev = 0;
+  BS_CUDA(cudaGetDevice(&dev));
+  BS_REQUIRE(dev >= 0 && dev < kMaxScratchDevices, BS_ERR_UNSUPPORTED, "device index %d", dev);
+  std::lock_guard<std::mutex> lock(g_scratch_mu);
+  if (g_scratch_addr[dev] == nullptr) {
+    void* ptr = nullptr;
+    BS_CUDA(cudaGetSymbolAddress(&ptr, g_static_scratch));
+    BS_REQUIRE(ptr != nullptr && ((uintptr_t)ptr & 255) == 0, BS_ERR_CUDA,
+               "bs_attn_fwd_static: scratch symbol address %p", ptr);
+    g_scratch_addr[dev] = (uint8_t*)ptr;
+  }
+  *out = g_scratch_addr[dev];
+  return BS_OK;
+}
+
+// [header | items | spans | groups | fill | tensor maps] as upload_tables (host_runtime.cpp) lays
+// them out, into host memory.  Everything the kernels read is written, the cursor as 0.
+void write_table_image(const bs::SchedTables& tb, const bs::WsLayout& L, uint8_t* img) {
+  memset(img, 0, L.total);
+  bs::SchedHeader* hd = reinterpret_cast<bs::SchedHeader*>(img);
+  hd->counter = 0;
+  hd->n_items = (int32_t)tb.items.size();
+  hd->n_spans = (int32_t)tb.spans.size();
+  hd->n_fill = (int32_t)tb.fill.size();
+  hd->n_groups = (int32_t)tb.groups.size();
+  hd->n_units = tb.n_units;
+  if (!tb.groups.empty())
+    memcpy(img + L.groups_off, tb.groups.data(), tb.groups.size() * sizeof(bs::Group));
+  if (!tb.items.empty())
+    memcpy(img + L.items_off, tb.items.data(), tb.items.size() * sizeof(bs::Item));
+  if (!tb.spans.empty())
+    memcpy(img + L.spans_off, tb.spans.data(), tb.spans.size() * sizeof(bs::Span));
+  if (!tb.fill.empty())
+    memcpy(img + L.fill_off, tb.fill.data(), tb.fill.size() * sizeof(bs::RowRange));
+  if (!tb.tmaps.empty()) memcpy(img + L.tmaps_off, tb.tmaps.data(), tb.tmaps.size());
+}
+
+}  // namespace
+
+extern "C" bs_status_t bs_attn_fwd_static(const bs_attn_shape_t* shape, const void* Q, const void* K,
+                                          const void* V, const bs_seg_t* segs, int32_t n_segs,
+                                          int32_t out_row_begin, int32_t out_row_end, void* O,
+                                          float* LSE, void* stream, float* dQ_acc_clear) {
+  bs_status_t rc = bs::validate_shape(shape, "bs_attn_fwd_static");
+  if (rc != BS_OK) return rc;
+  BS_REQUIRE(Q && K && V && O && LSE, BS_ERR_INVALID_ARG, "bs_attn_fwd_static: null tensor pointer");
+  BS_REQUIRE(n_segs >= 0 && (segs || n_segs == 0), BS_ERR_INVALID_ARG,
+             "bs_attn_fwd_static: bad segs");
+  BS_REQUIRE(0 <= out_row_begin && out_row_begin <= out_row_end && out_row_end <= shape->q_rows,
+             BS_ERR_INVALID_ARG, "bs_attn_fwd_static: output rows [%d,%d) outside [0,%d)",
+             out_row_begin, out_row_end, shape->q_rows);
+  BS_REQUIRE(((uintptr_t)O & 15) == 0, BS_ERR_INVALID_ARG,
+             "bs_attn_fwd_static: O not 16-byte aligned");
+  BS_REQUIRE(((uintptr_t)dQ_acc_clear & 15) == 0, BS_ERR_INVALID_ARG,
+             "bs_attn_fwd_static: dQ_acc_clear not 16-byte aligned");
+  if (out_row_end == out_row_begin) return BS_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  // As in bs_attn_fwd, everything that can fail on an argument comes before the first enqueue.
+  bs::SchedTables tb;
+  rc = bs::build_fwd_tables(segs, n_segs, shape->q_rows, shape->kv_rows, out_row_begin, out_row_end,
+                            shape->n_q_heads, &tb);
+  if (rc != BS_OK) return rc;
+  const bs::WsLayout L =
+      bs::ws_layout(tb.items.size(), tb.spans.size(), tb.groups.size(), tb.fill.size(),
+                    tb.clip_span_rows.size() * bs::kTensorMapBytes);
+  BS_REQUIRE(L.total <= kStaticScratchBytes, BS_ERR_WORKSPACE,
+             "bs_attn_fwd_static: the work list of this call needs %zu bytes of scratch, the "
+             "library's static scratch holds %zu (BS_ATTN_STATIC_SCRATCH_BYTES); use bs_attn_fwd "
+             "with a caller workspace",
+             L.total, kStaticScratchBytes);
+  rc = bs::check_device();
+  if (rc != BS_OK) return rc;
+  uint8_t* wsb = nullptr;
+  rc = static_scratch_address(&wsb);
+  if (rc != BS_OK) return rc;
+  const int D = shape->head_dim;
+  rc = bs::append_clipped_maps(&tb, 0, 1, tb.clip_span_rows, V, D, shape->n_kv_heads,
+                               shape->kv_row_stride);
+  if (rc != BS_OK) return rc;
+  CUtensorMap tmQ, tmK, tmV, tmZ;
+  rc = bs::make_tensor_map_3d(&tmQ, Q, 2, D, shape->n_q_heads, shape->q_rows, shape->q_row_stride,
+                              64, bs::kTile, 128);
+  if (rc != BS_OK) return rc;
+  rc = bs::make_tensor_map_3d(&tmK, K, 2, D, shape->n_kv_heads, shape->kv_rows,
+                              shape->kv_row_stride, 64, bs::kTile, 128);
+  if (rc != BS_OK) return rc;
+  rc = bs::make_tensor_map_3d(&tmV, V, 2, D, shape->n_kv_heads, shape->kv_rows,
+                              shape->kv_row_stride, 64, bs::kTile, 128);
+  if (rc != BS_OK) return rc;
+  rc = bs::make_tensor_map_3d(&tmZ, dQ_acc_clear ? (const void*)dQ_acc_clear : Q, 4, D,
+                              shape->n_q_heads, out_row_end, (int64_t)shape->n_q_heads * D, 32, 64, 0);
+  if (rc != BS_OK) return rc;
+  std::vector<uint8_t> img;  // host heap
+  try {
+    img.resize((L.total + kChunkBytes - 1) / kChunkBytes * kChunkBytes);
+  } catch (const std::bad_alloc&) {
+    return bs::fail(BS_ERR_HOST_OOM, "bs_attn_fwd_static: out of host memory (%zu bytes)", L.total);
+  }
+  write_table_image(tb, L, img.data());
+
+  // Tables -> scratch, a chunk per launch, by value: the launch copies the chunk into the
+  // parameter buffer, so `img` is dead when the loop ends.  Every byte the kernels below read
+  // (the cursor at offset 0 included) is rewritten, whatever the previous call left.
+  for (size_t off = 0; off < L.total; off += kChunkBytes) {
+    const size_t n = L.total - off < (size_t)kChunkBytes ? L.total - off : (size_t)kChunkBytes;
+    static_scratch_upload_kernel<<<1, kChunkBytes / 16, 0, st>>>(
+        *reinterpret_cast<const TableChunk*>(img.data() + off),
+        reinterpret_cast<uint4*>(wsb + off), (int)(n / 16));
+    BS_CUDA(cudaGetLastError());
+    bs::count_launch();
+  }
+  rc = bs::launch_fill_rows((const int2*)(wsb + L.fill_off), (int)tb.fill.size(), tb.max_fill_rows,
+                            O, nullptr, LSE, shape->n_q_heads, shape->head_dim, shape->q_row_stride,
+                            shape->lse_head_stride, st);
+  if (rc != BS_OK) return rc;
+  if (dQ_acc_clear != nullptr) {
+    const size_t row_bytes = (size_t)shape->n_q_heads * D * sizeof(float);
+    for (const bs::RowRange& f : tb.fill)
+      BS_CUDA(cudaMemsetAsync((uint8_t*)dQ_acc_clear + (size_t)f.begin * row_bytes, 0,
+                              (size_t)(f.end - f.begin) * row_bytes, st));
+  }
+  if (tb.items.empty()) return BS_OK;
+
+  FwdParams p;
+  p.clear_acc = dQ_acc_clear != nullptr;
+  p.wide_stores = ((uintptr_t)O & 31) == 0 && (shape->q_row_stride * 2) % 32 == 0 && (D * 2) % 32 == 0;
+  p.sv = bs::make_sched_view(wsb, L, tb, shape->n_q_heads);
+  p.n_q_heads = shape->n_q_heads;
+  p.group = shape->n_q_heads / shape->n_kv_heads;
+  p.q_rows = shape->q_rows;
+  const float scale = shape->softmax_scale > 0.f ? shape->softmax_scale : 1.f / sqrtf((float)D);
+  p.scale_log2 = scale * 1.4426950408889634f;
+  p.O = (__nv_bfloat16*)O;
+  p.LSE = LSE;
+  p.o_row_stride = shape->q_row_stride;
+  p.lse_head_stride = shape->lse_head_stride;
+  const int grid = tb.n_units < bs::sm_count() ? tb.n_units : bs::sm_count();
+  if (D == 128) {
+    rc = bs::set_max_smem_once((const void*)attn_fwd_kernel<128>, FwdSmem<128>::kAlloc, 0);
+    if (rc != BS_OK) return rc;
+    attn_fwd_kernel<128><<<grid, kFwdThreads, FwdSmem<128>::kAlloc, st>>>(tmQ, tmK, tmV, tmZ, p);
+  } else {
+    rc = bs::set_max_smem_once((const void*)attn_fwd_kernel<64>, FwdSmem<64>::kAlloc, 1);
+    if (rc != BS_OK) return rc;
+    attn_fwd_kernel<64><<<grid, kFwdThreads, FwdSmem<64>::kAlloc, st>>>(tmQ, tmK, tmV, tmZ, p);
+  }
+  BS_CUDA(cudaGetLastError());
+  bs::count_launch();
+  return BS_OK;
+}
