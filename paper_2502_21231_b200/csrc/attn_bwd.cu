@@ -339,6 +339,19 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const CUtensorMap* mQ = qclip ? clips_q + 2 * wk.sp.clip : &tmQ;
         const CUtensorMap* mDO = qclip ? mQ + 1 : &tmDO;
         const int own_q = qclip ? 1 + wk.sp.clip % 31 : 0;
+        // -lse*log2e (-inf for rows outside the query range) and -delta*scale: fetched BEFORE the
+        // wait for the stage (the producer runs ahead and sits in that wait), so that the ~800
+        // cycles of L2 latency are not in front of this iteration's dO request
+        float lse_v[kTile / 32], delta_v[kTile / 32];
+#pragma unroll
+        for (int k = 0; k < kTile / 32; ++k) {
+          const int c = lane + 32 * k;
+          const bool ok = wk.qi * kTile + c < wk.sp.len;
+          const int64_t idx = (int64_t)h * p.lse_head_stride + qrow + c;
+          // negated, so that the compute warps fold them in with one packed FMA each
+          lse_v[k] = ok ? -__ldg(p.LSE + idx) * 1.4426950408889634f : -CUDART_INF_F;
+          delta_v[k] = ok ? -__ldg(p.delta + idx) * p.scale : 0.f;
+        }
         mbar_wait(&q_empty[st], ((it_n >> 1) & 1) ^ 1);
         if (lane == own_q) {
           mbar_arrive_expect_tx(&q_full[st], L::kTileBytes);
@@ -346,14 +359,10 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tma_load_3d(smem + L::kQOff + st * L::kTileBytes + half * (kTile * 128), mQ,
                         &q_full[st], half * 64, h, qrow);
         }
-        // -lse*log2e (-inf for rows outside the query range) and -delta*scale
-        for (int c = lane; c < kTile; c += 32) {
-          const int a = wk.qi * kTile + c;
-          const bool ok = a < wk.sp.len;
-          const int64_t idx = (int64_t)h * p.lse_head_stride + qrow + c;
-          // negated, so that the compute warps fold them in with one packed FMA each
-          lse_s[st * kTile + c] = ok ? -p.LSE[idx] * 1.4426950408889634f : -CUDART_INF_F;
-          delta_s[st * kTile + c] = ok ? -p.delta[idx] * p.scale : 0.f;
+#pragma unroll
+        for (int k = 0; k < kTile / 32; ++k) {
+          lse_s[st * kTile + lane + 32 * k] = lse_v[k];
+          delta_s[st * kTile + lane + 32 * k] = delta_v[k];
         }
         mbar_arrive(&q_full[st]);
         if (lane == own_q) {
