@@ -271,7 +271,9 @@ bs_status_t bs_attn_fwd(const bs_attn_shape_t* shape, const void* Q, const void*
  * (no cudaMalloc / cudaFree / cudaHostAlloc, no allocating library routine; host heap only for
  * the work list): the tables reach the scratch as kernel PARAMETERS of small copy kernels
  * (3584 bytes per launch), so nothing is read from host memory after the call returns and the
- * host never waits for the stream.
+ * host never waits for the stream; a call can be captured into a CUDA graph (after one plain
+ * call on the device, which sets kernel attributes and resolves the scratch address) as long as
+ * the tensors it was captured with stay where they are.
  *   Limit: the call's tables must fit the array.  A call fits whenever
  * bs_attn_workspace_bytes(shape, n_segs, 0, &b) gives b <= BS_ATTN_STATIC_SCRATCH_BYTES (an
  * upper bound; the exact size is checked); otherwise BS_ERR_WORKSPACE with both sizes in

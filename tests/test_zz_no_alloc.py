@@ -151,3 +151,24 @@ def test_static_scratch_rejects_work_lists_beyond_its_size():
     assert bool((O2.float() == 0).all()) and float(L2.abs().max()) < 1e-3
     assert torch.equal(O2.view(torch.int16), O3.view(torch.int16))
     assert torch.equal(L2.view(torch.int32), L3.view(torch.int32))
+
+
+def test_static_scratch_forward_replays_from_a_cuda_graph():
+    """The call enqueues kernels whose inputs travel as kernel parameters (tables included) and
+    allocates nothing, so a captured launch can be replayed: capture one call of every ring step
+    (after a plain warm-up call: first use sets kernel attributes and resolves the scratch
+    address), clear the outputs, replay twice, compare with the existing path."""
+    ca, _ = _cases()
+    ca.launch("ref")
+    ca.launch("static")
+    torch.cuda.synchronize()
+    ca.reset("static")
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        ca.launch("static")
+    torch.cuda.synchronize()
+    for rnd in range(2):
+        ca.reset("static")
+        graph.replay()
+        torch.cuda.synchronize()
+        ca.compare(f"graph replay {rnd}, A")
