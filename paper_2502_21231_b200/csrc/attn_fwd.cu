@@ -222,7 +222,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
   if (warp == kTmaWarp && lane == 0) {
     *reinterpret_cast<uint32_t*>(smem + L::kLockOff) = 0;
-    sched_ring_init(sched, 4 * kTile + 3);  // 512 softmax threads + 2 MMA lanes + the TMA lane
+    sched_ring_init(sched, 4 * kTile / 32 + 3);  // 16 softmax warps + 2 MMA lanes + the TMA lane
     for (int t = 0; t < 2; ++t) {
       mbar_init(&q_full[t], 1);
       mbar_init(&q_empty[t], 1);
@@ -456,7 +456,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     UnitConsumer cons{sched};
     Unit u;
     int un = -1;
-    while (cons.next(&u)) {
+    while (cons.next_warp(&u, 0xffffffffu, 0)) {
       ++un;
       if (r == 0 && hf == 0) UTRACE(t, 0, un);
       const Item& it = u.item;
