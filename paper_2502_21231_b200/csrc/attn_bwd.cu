@@ -237,7 +237,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     __trap();
   }
   if (warp == 9 && lane == 0) {
-    sched_ring_init(sched, kComputeThreads + 2 + kTile);  // compute + MMA lane + TMA lane + drain WG
+    // arrivals per unit: one per compute warp, the MMA lane, the TMA lane, one per drain warp
+    sched_ring_init(sched, kComputeThreads / 32 + 2 + kTile / 32);
     mbar_init(k_full, 1);
     mbar_init(k_empty, 1);
     mbar_init(v_full, 1);
@@ -481,7 +482,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint32_t it_n = 0;
     UnitConsumer cons{sched};
     Unit u;
-    while (cons.next(&u)) {
+    while (cons.next_arrive_once(&u)) {
       const int g = u.head;
       BwdWalker wk;
       wk.init(p.sv.spans, u, p.group);
@@ -530,7 +531,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint32_t item_n = 0, it_n = 0;
     UnitConsumer cons{sched};
     Unit u;
-    while (cons.next(&u)) {
+    while (cons.next_arrive_once(&u)) {
       const Item& it = u.item;
       const int g = u.head;
       const int b = it.local0 + r;  // key index inside its range

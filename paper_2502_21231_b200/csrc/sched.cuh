@@ -157,6 +157,23 @@ struct UnitConsumerT {  // every consuming thread
     ++n;
     return w >= 0;
   }
+  // Converged warp, every lane waits for the slot itself (no extra hop on the way in), one
+  // arrival per warp on the way out.
+  __device__ __forceinline__ bool next_arrive_once(Unit* u) {
+    const uint32_t slot = n % kSlots, ph = (n / kSlots) & 1;
+    ptx::mbar_wait(&r->full[slot], ph);
+    const int32_t w = r->unit[slot];
+    if (w >= 0) {
+      u->item = r->item[slot];
+      u->head = r->head[slot];
+      u->sp[0] = r->sp[slot][0];
+      u->sp[1] = r->sp[slot][1];
+    }
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) ptx::mbar_arrive(&r->empty[slot]);
+    ++n;
+    return w >= 0;
+  }
   // Wait for slot n and read it without consuming it (lanes 1-31 of a warp whose lane 0
   // consumes for the warp afterwards).
   __device__ __forceinline__ void wait_peek(Unit* u) const {
