@@ -325,6 +325,8 @@ def run_ours(args, rank, world, local_rank):
         pk = peaks()
         nb = lambda t: t.numel() * t.element_size()  # noqa: E731
         merge = bench_merge(B, torch, pk)
+        red_dram = bench_reduce_probe(B, torch, acc)            # 512 MiB: every line misses L2
+        red_l2 = bench_reduce_probe(B, torch, acc[:4096])       # 64 MiB: the accumulator stays in L2
         xent = bench_softmax_xent(B, torch, pk)
         ring = bench_ring_steps(B, torch, workloads, pk)
         full = bench_full_configs(B, torch, workloads, pk)
@@ -348,6 +350,7 @@ def run_ours(args, rank, world, local_rank):
         value = world * flops_step * args.steps / (ms * 1e-3) / 1e12
         sus = world * flops_step * n_sus / (ms_sus * 1e-3) / 1e12
         prep_bytes = rows * Hq * (4 * D + 4)          # reads O, dO; writes delta (dQ_acc cleared by fwd)
+        bwd_red_bytes = tile_area_ratio(w) * pairs / (128 * 128) * Hq * 128 * D * 4   # tile-blocks x 64 KB
         fin_bytes = rows * Hq * 6 * D                 # reads fp32 dQ_acc, writes bf16 dQ
         # The driver keeps the contract keys of this line and the END of stdout: the long replay
         # records come first, what explains the headline (kernels, sustained, merge) sits inside
@@ -391,6 +394,16 @@ def run_ours(args, rank, world, local_rank):
                                        if pk["tflops_sustained"] else None,
                                        "frac_of_burst_peak": round(sus / world / pk["tflops"], 4),
                                        "sm_mhz_median": sampler.median_between(t_sus0, t_sus1)},
+                         # the backward's other ceiling: every computed 128 x 128
+                         # tile-block adds 128 x D fp32 of partial dQ into dQ_acc in the L2 atomic
+                         # units; the probes are that traffic alone (bs_reduce_probe), one CTA per SM,
+                         # units, L2-resident (64 MiB) and not (the whole 512 MiB accumulator)
+                         "l2_reduce": {"bytes_per_launch": int(bwd_red_bytes),
+                                       "achieved_gbs": round(bwd_red_bytes / t_bwd / 1e6, 1),
+                                       "probe_all_miss_gbs": round(red_dram, 1),
+                                       "probe_l2_resident_gbs": round(red_l2, 1),
+                                       "frac_of_all_miss_probe": round(bwd_red_bytes / t_bwd / 1e6 / red_dram, 4),
+                                       "frac_of_l2_resident_probe": round(bwd_red_bytes / t_bwd / 1e6 / red_l2, 4)},
                          "merge_gbs": {k: {"gbs": v["gbs"], "of_n_to_1_probe": v["frac_of_n_to_1_probe"],
                                                "of_measured_copy": v["frac_of_measured_copy"]}
                                            for k, v in merge["by_config"].items()}},
@@ -459,6 +472,23 @@ def bench_merge(B, torch, pk):
             "roofline": {"bound": "hbm", "achieved": c3["gbs"], "peak": pk["hbm"], "unit": "GB/s",
                          "frac": c3["gbs"] / pk["hbm"], "frac_of_nominal_8000": c3["gbs"] / 8000.0,
                          "traffic": ncu_traffic("lse_merge_kernel")}}
+
+
+def bench_reduce_probe(B, torch, acc):
+    """bs_reduce_probe: GB/s of fp32 reduce-adds (TMA boxes of 16 KB into `acc`, one CTA per SM, the
+    backward's own instruction and box shape) with nothing else running."""
+    boxes = 256
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    for _ in range(3):
+        B.reduce_probe(acc, boxes)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    it = 10
+    a.record()
+    for _ in range(it):
+        B.reduce_probe(acc, boxes)
+    b.record()
+    b.synchronize()
+    return n_sm * boxes * 16384 * it / (a.elapsed_time(b) * 1e-3) / 1e9
 
 
 def tile_area_ratio(w):

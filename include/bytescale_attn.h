@@ -350,6 +350,19 @@ bs_status_t bs_softmax_xent(const void* logits, const int32_t* labels, int32_t n
 bs_status_t bs_hbm_probe(int32_t n_in, const void* const* in, void* out, void* sink,
                          size_t bytes_per_stream, void* stream);
 
+/* Measurement aid for the backward's roofline: bs_attn_bwd adds every 128 x 128
+ * tile-block's partial dQ - 64 KB of fp32 at head_dim 128 - into dQ_acc with TMA reduce-adds that
+ * the L2 atomic units execute ("dQ_acc ... accumulated across steps", see bs_attn_bwd).  This call
+ * issues only such reduce boxes (the same instruction, box shape and tensor map; one CTA per SM,
+ * two boxes in flight each; the boxes hold zeros, so acc is unchanged): boxes_per_cta boxes of
+ * 128 rows x 32 columns = 16 KB per CTA.  Timed by the caller, it gives the fp32 reduce-add rate
+ * the device sustains with nothing else running, which bench.py reports the backward's own
+ * reduction traffic against.  acc: device, fp32 [rows][n_heads][head_dim] dense, 16-byte aligned;
+ * rows a multiple of 128, head_dim a multiple of 32 (<= 256).  Errors: INVALID_ARG, UNSUPPORTED,
+ * CUDA.  Asynchronous on stream. */
+bs_status_t bs_reduce_probe(float* acc, int32_t rows, int32_t n_heads, int32_t head_dim,
+                            int32_t boxes_per_cta, void* stream);
+
 /* Number of kernels this library has launched on the calling thread since the last reset
  * (bench.py's "gpu_launches"). */
 int64_t bs_launch_count(void);

@@ -121,6 +121,7 @@ lib.bs_attn_bwd_finish.argtypes = [_P(Shape), _vp, _vp, _vp]
 lib.bs_lse_merge.argtypes = [_i32, _P(_vp), _P(_vp), _P(Shape), _i32, _i32, _vp, _vp, _vp]
 lib.bs_softmax_xent.argtypes = [_vp, _vp, _i32, _i32, _i64, ctypes.c_float, _vp, _vp, _vp]
 lib.bs_hbm_probe.argtypes = [_i32, _P(_vp), _vp, _vp, _sz, _vp]
+lib.bs_reduce_probe.argtypes = [_vp, _i32, _i32, _i32, _i32, _vp]
 lib.bs_launch_count.restype = _i64
 lib.bs_launch_count_reset.restype = None
 
@@ -133,7 +134,7 @@ EXPORTS = ["bs_status_string", "bs_last_error", "bs_version", "bs_plan", "bs_pla
            "bs_balance_exec_times", "bs_balance_makespan", "bs_balance_n_microbatches",
            "bs_balance_microbatch", "bs_balance_destroy", "bs_attn_workspace_bytes", "bs_attn_fwd",
            "bs_attn_bwd_prep", "bs_attn_bwd", "bs_attn_bwd_finish", "bs_lse_merge", "bs_softmax_xent",
-           "bs_hbm_probe", "bs_attn_fwd_static",
+           "bs_hbm_probe", "bs_attn_fwd_static", "bs_reduce_probe",
            "bs_launch_count", "bs_launch_count_reset"]
 
 
@@ -322,6 +323,12 @@ def hbm_probe(ins, out, sink):
     arr = (_vp * n)(*[t.data_ptr() for t in ins])
     _check(lib.bs_hbm_probe(n, arr, _ptr(out), _ptr(sink), ins[0].numel() * ins[0].element_size(),
                             _stream()), "bs_hbm_probe")
+
+
+def reduce_probe(acc, boxes_per_cta):
+    """bs_reduce_probe on a torch device tensor acc fp32 [rows][heads][head_dim] (left unchanged)."""
+    rows, heads, hd = acc.shape
+    _check(lib.bs_reduce_probe(_ptr(acc), rows, heads, hd, boxes_per_cta, _stream()), "bs_reduce_probe")
 
 
 def launch_count():

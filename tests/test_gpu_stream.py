@@ -79,3 +79,21 @@ def test_bwd_prep_and_finish(nprng, rows, Hq, D):
     torch.cuda.synchronize()
     from conftest import f32_to_bf16_bits
     assert np.array_equal(U.to_bits(dQ), f32_to_bf16_bits(x.cpu().numpy()))
+
+
+def test_reduce_probe_leaves_the_accumulator_unchanged():
+    """bs_reduce_probe (measurement aid): fp32 reduce-add boxes of zeros into dQ_acc-shaped memory."""
+    import torch
+    from paper_2502_21231_b200 import binding as B
+    g = torch.Generator(device="cuda").manual_seed(3)
+    acc = torch.randn((1024, 3, 128), generator=g, device="cuda", dtype=torch.float32)
+    acc[5, 1, 7] = float("inf")
+    want = acc.clone()
+    B.reduce_probe(acc, 64)
+    B.reduce_probe(acc, 0)
+    torch.cuda.synchronize()
+    assert torch.equal(acc.view(torch.int32), want.view(torch.int32))
+    with pytest.raises(B.BsError):
+        B.reduce_probe(torch.zeros((100, 3, 128), device="cuda"), 4)       # rows not a multiple of 128
+    with pytest.raises(B.BsError):
+        B.reduce_probe(torch.zeros((128, 3, 48), device="cuda"), 4)        # head_dim not a multiple of 32
